@@ -1,0 +1,336 @@
+"""Pins for the oracle's shape layer (CPU only): depletant-colloid predicates (S16, S17), support
+functions and the convex-convex overlap test (S18), rotation algebra (S6, S19).
+
+References used are independent of the oracle's code path: Steiner volumes (closed form), dense point
+clouds of the solids (brute force), scipy's Rotation, closed-form contact distances, and an fp64 convex
+program (scipy SLSQP) for random pair poses.
+"""
+import ctypes as C
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy.optimize import minimize
+from scipy.spatial import cKDTree
+from scipy.spatial.transform import Rotation
+
+import oracle
+from oracle.binding import make_params
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _gold(key):
+    with open(os.path.join(GOLD, "paper_values.txt")) as f:
+        for line in f:
+            if line.startswith(key + " "):
+                return float(line.split()[1])
+    raise KeyError(key)
+
+
+HB = dict(shape="halfball", sigma_c=1.0, sigma_d=0.2, box_L=20.0, d_max_cap=0.1)
+SD = dict(shape="spherodisk", sigma_c=1.0, sigma_d=0.15, box_L=20.0, d_max_cap=0.1, disk_a=0.4, disk_s=0.1)
+SP = dict(shape="sphere", sigma_c=1.0, sigma_d=0.2, box_L=20.0, d_max_cap=0.1)
+
+
+def rand_quats(n, rng):
+    q = rng.standard_normal((n, 4))
+    q /= np.linalg.norm(q, axis=1, keepdims=True)
+    return q.astype(np.float32)
+
+
+def q_to_R(q):
+    """(w,x,y,z) -> scipy Rotation (scalar-last there)."""
+    q = np.asarray(q, np.float64)
+    return Rotation.from_quat(np.r_[q[1:], q[0]])
+
+
+def dep_overlap(params, quat, d):
+    p = make_params(**params)
+    q = np.ascontiguousarray(quat, np.float32)
+    d = np.ascontiguousarray(d, np.float32)
+    out = np.zeros(len(d), np.uint8)
+    oracle.lib().oracle_dep_overlap(C.byref(p), q.ctypes.data, d.ctypes.data, len(d), out.ctypes.data)
+    return out.astype(bool)
+
+
+def pair_overlap(params, rho, qA, qB):
+    p = make_params(**params)
+    rho = np.ascontiguousarray(np.atleast_2d(rho), np.float32)
+    qA = np.ascontiguousarray(np.atleast_2d(qA), np.float32)
+    qB = np.ascontiguousarray(np.atleast_2d(qB), np.float32)
+    out = np.zeros(len(rho), np.uint8)
+    oracle.lib().oracle_pair_overlap(C.byref(p), rho.ctypes.data, qA.ctypes.data, qB.ctypes.data, len(rho),
+                                     out.ctypes.data)
+    return out.astype(bool)
+
+
+def shape_cloud(params, n, rng):
+    """Dense fp64 point cloud of the solid in its body frame (volume + boundary points)."""
+    if params["shape"] == "halfball":
+        R = 0.5 * params["sigma_c"]
+        v = rng.standard_normal((n, 3))
+        v /= np.linalg.norm(v, axis=1, keepdims=True)
+        vol = v * (R * rng.random((n, 1)) ** (1 / 3))
+        vol[:, 2] = -np.abs(vol[:, 2])
+        dome = v * R
+        dome[:, 2] = -np.abs(dome[:, 2])
+        ang, rad = rng.random(n) * 2 * np.pi, R * np.sqrt(rng.random(n))
+        face = np.stack([rad * np.cos(ang), rad * np.sin(ang), np.zeros(n)], -1)
+        rim = np.stack([R * np.cos(ang), R * np.sin(ang), np.zeros(n)], -1)
+        return np.concatenate([vol, dome, face, rim])
+    a, s = params["disk_a"], params["disk_s"]
+    ang, rad = rng.random(n) * 2 * np.pi, a * np.sqrt(rng.random(n))
+    disk = np.stack([rad * np.cos(ang), rad * np.sin(ang), np.zeros(n)], -1)
+    disk[: n // 4, :2] *= (a / np.maximum(1e-12, np.linalg.norm(disk[: n // 4, :2], axis=1)))[:, None]   # rim
+    v = rng.standard_normal((n, 3))
+    v /= np.linalg.norm(v, axis=1, keepdims=True)
+    return np.concatenate([disk + s * v, disk + s * v * rng.random((n, 1))])
+
+
+# ----------------------------------------------------------------------------------- depletant tests
+@pytest.mark.parametrize("params,key", [(HB, "halfball_steiner_fraction"), (SD, "spherodisk_steiner_fraction")])
+def test_dilated_volume_steiner(olib, params, key):
+    """Fraction of insertion-ball samples that overlap the shape = Steiner volume / ball volume."""
+    n = 1000000
+    R = 0.5 * (params["sigma_c"] + params["sigma_d"])
+    d = np.zeros((n, 3), np.float32)
+    olib.oracle_ball_samples(3, 1, 0, 77, n, R, d.ctypes.data)
+    q = rand_quats(1, np.random.default_rng(5))[0]
+    frac = dep_overlap(params, q, d).mean()
+    want = _gold(key)
+    assert abs(frac - want) < 4.5 * math.sqrt(want * (1 - want) / n) + 2e-5
+
+
+def test_dilated_volume_sphere(olib):
+    n = 100000
+    d = np.zeros((n, 3), np.float32)
+    olib.oracle_ball_samples(3, 1, 0, 78, n, 0.6, d.ctypes.data)
+    assert dep_overlap(SP, [1, 0, 0, 0], d).mean() > 0.9999
+    assert not dep_overlap(SP, [1, 0, 0, 0], np.array([[0.6, 0.0, 0.0], [0.4, 0.4, 0.3]], np.float32)).any()
+
+
+def test_spherodisk_volume_formula():
+    import workloads
+    assert abs(workloads.spherodisk_volume(0.4, 0.1) - _gold("spherodisk_volume")) < 1e-6
+
+
+@pytest.mark.parametrize("params", [HB, SD])
+def test_dep_overlap_vs_point_cloud(params):
+    """Predicate == (distance from the depletant centre to the solid < r_d), by brute force."""
+    rng = np.random.default_rng(11)
+    cloud = shape_cloud(params, 150000, rng)
+    tree = cKDTree(cloud)
+    rd = 0.5 * params["sigma_d"]
+    q = rand_quats(1, rng)[0]
+    Rm = q_to_R(q)
+    pts_body = (rng.random((4000, 3)) - 0.5) * 1.5
+    dist, _ = tree.query(pts_body)
+    pts_world = Rm.apply(pts_body)
+    got = dep_overlap(params, q, pts_world)
+    band = 0.012                                    # cloud resolution
+    sure_in, sure_out = dist < rd - band, dist > rd + band
+    assert sure_in.sum() > 300 and sure_out.sum() > 300
+    assert got[sure_in].all()
+    assert not got[sure_out].any()
+
+
+# ----------------------------------------------------------------------------------- support function
+@pytest.mark.parametrize("params", [HB, SD])
+def test_support_is_argmax_over_cloud(olib, params):
+    rng = np.random.default_rng(12)
+    cloud = shape_cloud(params, 100000, rng)
+    p = make_params(**params)
+    for _ in range(40):
+        q = rand_quats(1, rng)[0]
+        n = (rng.standard_normal(3) * rng.choice([0.01, 1.0, 30.0])).astype(np.float32)
+        out = np.zeros(3, np.float32)
+        olib.oracle_support(C.byref(p), q.ctypes.data, n.ctypes.data, out.ctypes.data)
+        world = q_to_R(q).apply(cloud)
+        nn = n.astype(np.float64) / np.linalg.norm(n)
+        h_cloud = (world @ nn).max()
+        h = float(out.astype(np.float64) @ nn)
+        assert h >= h_cloud - 1e-5                  # no point of the solid lies beyond the support plane
+        assert h <= h_cloud + 0.01                  # and the support point is (nearly) attained by the cloud
+    # special directions
+    ident = np.array([1, 0, 0, 0], np.float32)
+    for n, want in (([0, 0, 1], None), ([0, 0, -1], None), ([1, 0, 0], None)):
+        out = np.zeros(3, np.float32)
+        nv = np.array(n, np.float32)
+        olib.oracle_support(C.byref(p), ident.ctypes.data, nv.ctypes.data, out.ctypes.data)
+        if params["shape"] == "halfball":
+            exp = {(0, 0, 1): 0.0, (0, 0, -1): 0.5, (1, 0, 0): 0.5}[tuple(n)]
+        else:
+            exp = {(0, 0, 1): 0.1, (0, 0, -1): 0.1, (1, 0, 0): 0.5}[tuple(n)]
+        assert abs(float(out @ nv) - exp) < 1e-6
+
+
+# ----------------------------------------------------------------------------------- pair overlap
+def quat_from_axis(z):
+    """Any quaternion whose body z axis is the given unit vector."""
+    z = np.asarray(z, np.float64) / np.linalg.norm(z)
+    r, _ = Rotation.align_vectors([z], [[0, 0, 1]])
+    x, y, zz, w = r.as_quat()
+    return np.array([w, x, y, zz], np.float32)
+
+
+def test_pair_overlap_closed_forms_spherodisk():
+    """S18: coaxial spherodisks overlap iff |dz| < 2s; coplanar iff centre distance < 2(a+s)."""
+    q = quat_from_axis([0, 0, 1])
+    for dz in np.linspace(0.05, 0.4, 36):
+        if abs(dz - 0.2) < 1e-3:
+            continue
+        assert pair_overlap(SD, [0, 0, dz], q, q)[0] == (dz < 0.2)
+        assert pair_overlap(SD, [0.3, 0, dz], q, q)[0] == (dz < 0.2)       # still face to face
+    for dx in np.linspace(0.8, 1.2, 41):
+        if abs(dx - 1.0) < 1e-3:
+            continue
+        assert pair_overlap(SD, [dx, 0, 0], q, q)[0] == (dx < 1.0)
+    # T configuration: B's axis along x, B's rim towards A's face: contact at dz = s + (a + s)
+    qx = quat_from_axis([1, 0, 0])
+    for dz in np.linspace(0.4, 0.8, 41):
+        if abs(dz - 0.6) < 1e-3:
+            continue
+        assert pair_overlap(SD, [0, 0, dz], q, qx)[0] == (dz < 0.6)
+    # tilted orientation-independent sanity: far apart never, coincident always
+    rng = np.random.default_rng(3)
+    qa, qb = rand_quats(200, rng), rand_quats(200, rng)
+    assert pair_overlap(SD, np.tile([0.0, 0.0, 0.0], (200, 1)), qa, qb).all()
+    assert not pair_overlap(SD, np.tile([1.0001, 0.0, 0.0], (200, 1)), qa, qb).any()
+    # closer than the thickness 2s the two always overlap, whatever the orientations
+    dirs = rng.standard_normal((200, 3))
+    dirs /= np.linalg.norm(dirs, axis=1, keepdims=True)
+    assert pair_overlap(SD, 0.19 * dirs, qa, qb).all()
+
+
+def test_pair_overlap_closed_forms_halfball():
+    """S18/S15: solid {|x|<=R, x.a<=0}: dome towards -a, flat face through the centre with normal +a."""
+    up, dn = quat_from_axis([0, 0, 1]), quat_from_axis([0, 0, -1])
+    # domes facing each other along z: A's dome towards +z (a=-z), B above with dome towards -z (a=+z)
+    for d in np.linspace(0.8, 1.2, 41):
+        if abs(d - 1.0) < 1e-3:
+            continue
+        assert pair_overlap(HB, [0, 0, d], dn, up)[0] == (d < 1.0)
+    # flat faces facing each other with a gap h > 0: never
+    for h in (1e-3, 0.01, 0.1, 0.5):
+        assert not pair_overlap(HB, [0, 0, h], up, dn)[0]
+        assert not pair_overlap(HB, [0.3, 0.1, h], up, dn)[0]
+    # ... and interpenetrating when the gap is negative
+    for h in (-1e-3, -0.01, -0.1):
+        assert pair_overlap(HB, [0, 0, h], up, dn)[0]
+    # A's flat face (normal +z) against B's dome pointing down (a_B=+z): contact when d = R
+    for d in np.linspace(0.3, 0.7, 41):
+        if abs(d - 0.5) < 1e-3:
+            continue
+        assert pair_overlap(HB, [0, 0, d], up, up)[0] == (d < 0.5)
+    # side by side, same axis: the great half-discs touch at d = 2R
+    for d in np.linspace(0.8, 1.2, 41):
+        if abs(d - 1.0) < 1e-3:
+            continue
+        assert pair_overlap(HB, [d, 0, 0], up, up)[0] == (d < 1.0)
+    # back to back (flat faces outward): A dome +z? no: A a=+z has its dome towards -z; B below with a=-z
+    # has its dome towards +z -> domes facing, contact at 2R; while B ABOVE A (d>0) with a_B=-z: faces facing
+    for d in np.linspace(0.8, 1.2, 9):
+        if abs(d - 1.0) < 1e-3:
+            continue
+        assert pair_overlap(HB, [0, 0, -d], up, dn)[0] == (d < 1.0)
+
+
+def _gauge(params):
+    """fp64 convex gauge g(x) <= 0 inside the solid (body frame at origin, axis = body z)."""
+    if params["shape"] == "halfball":
+        R = 0.5 * params["sigma_c"]
+        return lambda b: max(np.linalg.norm(b) - R, b[2])
+    a, s = params["disk_a"], params["disk_s"]
+
+    def g(b):
+        rho = math.hypot(b[0], b[1])
+        return math.hypot(max(rho - a, 0.0), b[2]) - s
+    return g
+
+
+def _deepest_common_point(params, rho, qA, qB):
+    """min_x max(g_A(x), g_B(x)) by an epigraph convex program (SLSQP, several starts)."""
+    g = _gauge(params)
+    MA, MB = q_to_R(qA).as_matrix().T, q_to_R(qB).as_matrix().T     # space -> body
+    rho = np.asarray(rho, np.float64)
+    gA = lambda x: g(MA @ x)
+    gB = lambda x: g(MB @ (x - rho))
+    best = np.inf
+    for x0 in (0.5 * rho, 0.3 * rho + 0.03):
+        t0 = max(gA(x0), gB(x0))
+        res = minimize(lambda z: z[3], np.r_[x0, t0], method="SLSQP",
+                       constraints=[{"type": "ineq", "fun": lambda z: z[3] - gA(z[:3])},
+                                    {"type": "ineq", "fun": lambda z: z[3] - gB(z[:3])}],
+                       options={"ftol": 1e-12, "maxiter": 300})
+        x = res.x[:3]
+        best = min(best, max(gA(x), gB(x)))
+    return best
+
+
+@pytest.mark.parametrize("params", [HB, SD])
+def test_pair_overlap_vs_convex_program(params):
+    """Random poses inside the circumsphere range: MPR's verdict == sign of the fp64 convex program,
+    outside a contact band."""
+    rng = np.random.default_rng(21)
+    n = 60
+    dirs = rng.standard_normal((n, 3))
+    dirs /= np.linalg.norm(dirs, axis=1, keepdims=True)
+    lo = 0.15 if params["shape"] == "spherodisk" else 0.05
+    rho = (dirs * (lo + (1.0 - lo) * rng.random((n, 1)))).astype(np.float32)
+    qA, qB = rand_quats(n, rng), rand_quats(n, rng)
+    got = pair_overlap(params, rho, qA, qB)
+    n_in = n_out = 0
+    for k in range(n):
+        f = _deepest_common_point(params, rho[k], qA[k], qB[k])
+        if f < -2e-4:
+            assert got[k], (k, f)
+            n_in += 1
+        elif f > 2e-4:
+            assert not got[k], (k, f)
+            n_out += 1
+    assert n_in > 10 and n_out > 10
+
+
+def test_pair_overlap_symmetric_outside_band():
+    """Swapping the roles of A and B (rho -> -rho) gives the same verdict for generic poses."""
+    rng = np.random.default_rng(22)
+    n = 20000
+    dirs = rng.standard_normal((n, 3))
+    dirs /= np.linalg.norm(dirs, axis=1, keepdims=True)
+    rho = (dirs * (0.2 + 0.8 * rng.random((n, 1)))).astype(np.float32)
+    qA, qB = rand_quats(n, rng), rand_quats(n, rng)
+    for params in (HB, SD):
+        ab = pair_overlap(params, rho, qA, qB)
+        ba = pair_overlap(params, -rho, qB, qA)
+        assert (ab != ba).mean() < 2e-3            # only poses inside the 1e-5 contact band may differ
+        assert 0.15 < ab.mean() < 0.9
+
+
+def test_sphere_pair_overlap_exact():
+    q = np.array([1, 0, 0, 0], np.float32)
+    assert pair_overlap(SP, [0.999999, 0, 0], q, q)[0]
+    assert not pair_overlap(SP, [1.0, 0, 0], q, q)[0]              # S14: touching is not overlapping
+    assert not pair_overlap(SP, [0.6, 0.6, 0.6], q, q)[0]
+    assert pair_overlap(SP, [0.57, 0.57, 0.57], q, q)[0]
+
+
+# ----------------------------------------------------------------------------------- rotations
+def test_quat_axis_and_cayley_vs_scipy(olib):
+    rng = np.random.default_rng(31)
+    for _ in range(200):
+        q = rand_quats(1, rng)[0]
+        ax = np.zeros(3, np.float32)
+        olib.oracle_quat_axis(q.ctypes.data, ax.ctypes.data)
+        assert np.allclose(ax, q_to_R(q).apply([0, 0, 1]), atol=2e-6)
+        v = (rng.standard_normal(3) * 0.1).astype(np.float32)
+        out = np.zeros(4, np.float32)
+        olib.oracle_rotate_cayley(q.ctypes.data, v.ctypes.data, out.ctypes.data)
+        assert abs(np.linalg.norm(out.astype(np.float64)) - 1.0) < 3e-7
+        # (1,v)/sqrt(1+v^2) is the rotation by 2 atan|v| about v, applied on the left (space frame)
+        ang = 2.0 * math.atan(np.linalg.norm(v.astype(np.float64)))
+        dR = Rotation.from_rotvec(v.astype(np.float64) / np.linalg.norm(v) * ang)
+        want = (dR * q_to_R(q)).as_matrix()
+        got = q_to_R(out).as_matrix()
+        assert np.allclose(got, want, atol=5e-6)
