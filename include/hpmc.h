@@ -1,0 +1,153 @@
+/* hpmc.h -- C-ABI boundary of the B200 (sm_100a) implicit-depletant hard-particle Monte Carlo library.
+ *
+ * The library implements ONE thing: the checkerboard-parallel colloid trial move with implicit
+ * (ideal-gas) depletant insertion of arXiv 1508.07077 (Glaser, Karas, Glotzer).  Citations are line
+ * numbers of /root/reference/PAPER.md (L<n>) and the readings R-* listed in DESIGN.md.
+ *
+ *   move rule            Sec. III.B  L64-68, Fig. 2 L72, Eq. 5
+ *   insertion volume     Sec. III.C  L117, L156 (circumsphere of diameter d_colloid+d_depletant, new pose)
+ *   configurational bias Sec. III.D  L170-174, Eq. 16
+ *   checkerboard         Sec. III.E  L180
+ *
+ * Conventions
+ *   - All entry points are extern "C", take plain pointers and sizes, return 0 on success or a negative
+ *     hpmc_status; they never throw.  hpmc_last_error() gives the message of the last failure.
+ *   - "device" pointers are CUDA device pointers of the current device; "host" pointers are ordinary (or,
+ *     better, page-locked) host memory.  Every argument below says which.
+ *   - Poses: centre = float4 (x, y, z, unused) with 0 <= x,y,z < box_L; orientation = float4 unit
+ *     quaternion (w, x, y, z).  fp32 throughout (paper: "single precision", L232).
+ *   - Work is enqueued on the cudaStream_t given to hpmc_init and is asynchronous unless stated.
+ *   - There is no CPU fallback: without a CUDA device every call that touches the device fails with
+ *     HPMC_E_CUDA.
+ */
+#ifndef HPMC_H_
+#define HPMC_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hpmc_ctx hpmc_ctx; /* opaque, library-owned */
+
+typedef enum {
+  HPMC_SPHERE = 0,     /* sphere of diameter sigma_c */
+  HPMC_HALFBALL = 1,   /* {x: |x| <= sigma_c/2, x.z_body <= 0}: flat face through the pose centre, outward normal +z_body */
+  HPMC_SPHERODISK = 2  /* Minkowski sum of a flat disk (radius disk_a, normal z_body) and a ball (radius disk_s) */
+} hpmc_shape;
+
+typedef enum {
+  HPMC_OK = 0,
+  HPMC_E_BADARG = -1,            /* NULL pointer, N <= 0, box_L <= 0, negative density, n_trial > 65535 ... */
+  HPMC_E_GEOMETRY = -2,          /* fewer than 4 cells per axis: box too small for the interaction range */
+  HPMC_E_STATE = -3,             /* hpmc_sweep without hpmc_build_cells for the same (seed, step) */
+  HPMC_E_DMAX = -4,              /* d_max > d_max_cap given at init */
+  HPMC_E_CUDA = -5,              /* CUDA runtime error (message in hpmc_last_error) */
+  HPMC_E_NEIGHBOR_OVERFLOW = -6  /* more neighbours in range than the staging buffer holds (reported by the
+                                    next synchronising call; poses of that sweep are then invalid) */
+} hpmc_status;
+
+typedef struct {
+  int32_t shape;       /* hpmc_shape */
+  float sigma_c;       /* circumsphere diameter d_colloid: sphere diameter, 2 R_halfball, 2 (disk_a + disk_s) */
+  float disk_a;        /* spherodisk only */
+  float disk_s;        /* spherodisk only */
+  float sigma_d;       /* depletant diameter d_depletant (>= 0) */
+  float box_L;         /* edge of the cubic periodic box */
+  float d_max_cap;     /* largest d_max any later sweep will use; fixes the cell width
+                          w >= sigma_c + sigma_d + 2 d_max_cap (BASELINE.json north_star; L180) */
+} hpmc_params;
+
+/* All counters accumulate since init / hpmc_reset_counters. */
+typedef struct {
+  uint64_t trials_trans, accept_trans, trials_rot, accept_rot;
+  uint64_t rej_boundary;    /* new centre left the cell (L180 "not allowed to move outside their cells") */
+  uint64_t rej_hard;        /* overlap with another colloid (Eq. 5) */
+  uint64_t rej_depletant;   /* plain rule: a depletant overlapped the new pose only (L68, L72) */
+  uint64_t rej_cb;          /* configurational-bias rule: zero weight or u >= product (Eq. 16) */
+  uint64_t dep_drawn;       /* sum of N_d over moves that reached the depletant stage (L67) */
+  uint64_t dep_needed;      /* sum of (index of the first rejecting depletant + 1), or N_d if none: the
+                               sequential algorithm's work; identical in the oracle */
+  uint64_t dep_evaluated;   /* depletant positions the kernel actually generated (>= dep_needed) */
+  uint64_t cb_reinsertions; /* 2 n_trial per rejecting depletant handled (Sec. III.D) */
+  uint64_t philox_blocks;   /* Philox4x32-10 blocks computed (warp-uniform ones counted once) */
+} hpmc_counters_t;
+
+/* Per-particle outcome code of the last sweep (each particle is tried at most once per sweep). */
+enum { HPMC_OUT_NONE = 0, HPMC_OUT_ACCEPT = 1, HPMC_OUT_BOUNDARY = 2, HPMC_OUT_HARD = 3,
+       HPMC_OUT_DEPLETANT = 4, HPMC_OUT_CB = 5 };
+
+/* Create a context for N colloids.
+ *   d_pos4   device, N x float4, caller-owned, borrowed for the context's lifetime, updated IN PLACE by
+ *            hpmc_sweep.  NULL: the library allocates its own pose buffers (use hpmc_upload/hpmc_download).
+ *   d_quat4  device, N x float4 (w,x,y,z), same ownership; may be NULL for spheres.  Must be NULL iff
+ *            d_pos4 is NULL.
+ *   cuda_stream  a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream), or NULL for the default.
+ * Cell grid (R-1, L180): n_c = largest even integer <= box_L / (sigma_c + sigma_d + 2 d_max_cap) per axis,
+ * n_c >= 4 else HPMC_E_GEOMETRY.  Cell arrays, tables, counters are library-owned device memory. */
+int hpmc_init(hpmc_ctx** out, const hpmc_params* p, int64_t N, float* d_pos4, float* d_quat4, void* cuda_stream);
+
+/* Free everything the library owns.  Caller-owned pose buffers are left alone.  Synchronises the stream. */
+void hpmc_destroy(hpmc_ctx* ctx);
+
+/* Cell-list build, step a2: draws this sweep's grid shift from Philox(seed, step) ("grid lines are randomly
+ * shifted", L180), bins the centres, lists the occupants of every cell in ascending particle id and writes the
+ * cell-ordered pose copy.  Call once before every hpmc_sweep with the same (seed, step).  Asynchronous. */
+int hpmc_build_cells(hpmc_ctx* ctx, uint32_t seed, uint32_t step);
+
+/* One sweep = the 8 checkerboard sub-lattice passes in a Philox-permuted order (L180), steps a3-a10.  In every
+ * non-empty active cell one colloid gets a trial move: translation uniform in [-d_max, d_max]^3, or (if
+ * a_max > 0, with probability 1/2) a Cayley rotation with parameter vector uniform in the ball of radius a_max.
+ *   n_R      depletant reservoir number density (fugacity z_p, L214); 0 = plain hard-particle MC
+ *   n_trial  0 = plain rule (L68); > 0 = configurational bias with n_trial reinsertions each way (Eq. 16)
+ * Requires hpmc_build_cells(seed, step) before it, else HPMC_E_STATE; d_max <= d_max_cap else HPMC_E_DMAX.
+ * Asynchronous; poses are updated in place. */
+int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_max, float a_max, int32_t n_trial);
+
+/* n_sweeps x (hpmc_build_cells + hpmc_sweep) with step = step0, step0+1, ...  Asynchronous. */
+int hpmc_run(hpmc_ctx* ctx, uint32_t seed, uint32_t step0, int64_t n_sweeps, double n_R, float d_max, float a_max,
+             int32_t n_trial);
+
+/* Synchronise the stream and copy the counters to host_out (host).  Does not reset them.  Reports a pending
+ * HPMC_E_NEIGHBOR_OVERFLOW. */
+int hpmc_counters(hpmc_ctx* ctx, hpmc_counters_t* host_out);
+int hpmc_reset_counters(hpmc_ctx* ctx);
+
+/* Copy the outcome codes of the last sweep into d_outcome (device, N bytes, caller-owned).  Asynchronous. */
+int hpmc_outcomes(hpmc_ctx* ctx, uint8_t* d_outcome);
+
+/* Grid geometry chosen at init: cells per axis and cell width. */
+int hpmc_grid(hpmc_ctx* ctx, int32_t* n_c, float* w);
+
+/* Debug / parity: copy the cell list of the last hpmc_build_cells into caller-owned DEVICE buffers
+ * (cell_start: n_c^3 + 1 uint32; cell_pid: N uint32) and the grid shift into host_shift3 (host, 3 floats).
+ * Synchronises the stream. */
+int hpmc_cells(hpmc_ctx* ctx, uint32_t* d_cell_start, uint32_t* d_cell_pid, float* host_shift3);
+
+/* Host-buffer path (end-to-end measurements; library-owned pose buffers or borrowed ones alike).
+ * hpmc_upload: host -> device copy of N x float4 centres (and orientations unless NULL).
+ * hpmc_download: device -> host copy of centres, orientations and outcome codes (any may be NULL).
+ * hpmc_step_host: upload, hpmc_build_cells, hpmc_sweep, download, then synchronise: one whole step with the
+ * host<->device traffic inside it. */
+int hpmc_upload(hpmc_ctx* ctx, const float* host_pos4, const float* host_quat4);
+int hpmc_download(hpmc_ctx* ctx, float* host_pos4, float* host_quat4, uint8_t* host_outcome);
+int hpmc_step_host(hpmc_ctx* ctx, float* host_pos4, float* host_quat4, uint8_t* host_outcome, uint32_t seed,
+                   uint32_t step, double n_R, float d_max, float a_max, int32_t n_trial);
+
+/* Number of kernel launches the library has enqueued since init (for bench.py's gpu_launches). */
+int64_t hpmc_launch_count(hpmc_ctx* ctx);
+
+/* Event timing of the move kernel (the dominant kernel): while enabled, every move-kernel launch is bracketed
+ * by CUDA events on the context's stream; hpmc_move_kernel_ms synchronises and returns the accumulated
+ * milliseconds and launch count since enabling. */
+int hpmc_time_move_kernel(hpmc_ctx* ctx, int32_t enable);
+int hpmc_move_kernel_ms(hpmc_ctx* ctx, double* ms_total, int64_t* launches);
+
+/* Message of the last error on this context (or of the last failed hpmc_init if ctx is NULL). */
+const char* hpmc_last_error(hpmc_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HPMC_H_ */

@@ -1,0 +1,134 @@
+// cells.cuh -- step a2: cell-list build (K-A).  PAPER.md L180 (checkerboard grid, "grid lines are randomly
+// shifted"); BASELINE.json north_star (2).  Deterministic layout: occupants of a cell in ascending particle id,
+// cells in ascending linear index (ix fastest), so a row of 3 x-neighbour cells is one contiguous span.
+//   k_bin_count   cell id + arrival rank per particle (atomic), counts per cell
+//   k_scan_*      exclusive scan of the counts -> cell_start            (3 small kernels)
+//   k_fill        scatter particle ids to cell_start[c] + rank
+//   k_sort_write  per cell: sort its few ids ascending (removes the atomics' arrival order) and write the
+//                 cell-ordered pose copy cpos = (x,y,z,pid) and, for anisotropic shapes, caxis = body z axis
+#pragma once
+#include <cstdint>
+#include "geometry.cuh"
+
+namespace hpmc {
+
+__global__ void __launch_bounds__(256) k_bin_count(const float4* __restrict__ pos, int N, Geo g, float sx, float sy,
+                                                   float sz, uint32_t* __restrict__ cid, uint32_t* __restrict__ rank,
+                                                   uint32_t* __restrict__ counts) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const float4 p = pos[i];
+  const int ix = cell_axis(g, p.x, sx), iy = cell_axis(g, p.y, sy), iz = cell_axis(g, p.z, sz);
+  const uint32_t c = ((uint32_t)iz * g.nc + iy) * g.nc + ix;
+  cid[i] = c;
+  rank[i] = atomicAdd(&counts[c], 1u);
+}
+
+constexpr int SCAN_THREADS = 256;
+constexpr int SCAN_ITEMS = 8;
+constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
+
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* s_warp, uint32_t& block_total) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  uint32_t incl = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += t;
+  }
+  if (lane == 31) s_warp[wid] = incl;
+  __syncthreads();
+  if (wid == 0) {
+    uint32_t w = (lane < (int)(blockDim.x >> 5)) ? s_warp[lane] : 0u;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, w, o);
+      if (lane >= o) w += t;
+    }
+    s_warp[lane] = w;   // inclusive over warps
+  }
+  __syncthreads();
+  const uint32_t warp_off = wid ? s_warp[wid - 1] : 0u;
+  block_total = s_warp[(blockDim.x >> 5) - 1];
+  return warp_off + incl - v;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_tiles(const uint32_t* __restrict__ counts, int n,
+                                                             uint32_t* __restrict__ tile_sums) {
+  __shared__ uint32_t s_warp[32];
+  const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+  uint32_t s = 0;
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) s += (base + k < n) ? counts[base + k] : 0u;
+  uint32_t total;
+  block_exclusive_scan(s, s_warp, total);
+  if (threadIdx.x == 0) tile_sums[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(1024) k_scan_top(uint32_t* __restrict__ tile_sums, int ntiles) {
+  __shared__ uint32_t s_warp[32];
+  uint32_t carry = 0;
+  for (int base = 0; base < ntiles; base += 1024) {
+    const int i = base + threadIdx.x;
+    const uint32_t v = i < ntiles ? tile_sums[i] : 0u;
+    uint32_t total;
+    const uint32_t ex = block_exclusive_scan(v, s_warp, total);
+    if (i < ntiles) tile_sums[i] = carry + ex;
+    carry += total;
+    __syncthreads();
+  }
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(const uint32_t* __restrict__ counts, int n,
+                                                             const uint32_t* __restrict__ tile_sums,
+                                                             uint32_t* __restrict__ cell_start) {
+  __shared__ uint32_t s_warp[32];
+  const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+  uint32_t v[SCAN_ITEMS], s = 0;
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) { v[k] = (base + k < n) ? counts[base + k] : 0u; s += v[k]; }
+  uint32_t total;
+  uint32_t run = tile_sums[blockIdx.x] + block_exclusive_scan(s, s_warp, total);
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) {
+    if (base + k < n) cell_start[base + k] = run;
+    run += v[k];
+    if (base + k == n - 1) cell_start[n] = run;
+  }
+}
+
+__global__ void __launch_bounds__(256) k_fill(const uint32_t* __restrict__ cid, const uint32_t* __restrict__ rank,
+                                              const uint32_t* __restrict__ cell_start, int N,
+                                              uint32_t* __restrict__ cell_pid) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  cell_pid[cell_start[cid[i]] + rank[i]] = (uint32_t)i;
+}
+
+template <bool ANISO>
+__global__ void __launch_bounds__(256) k_sort_write(const uint32_t* __restrict__ cell_start, int ncell,
+                                                    uint32_t* __restrict__ cell_pid, const float4* __restrict__ pos,
+                                                    const float4* __restrict__ quat, float4* __restrict__ cpos,
+                                                    float4* __restrict__ caxis) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncell) return;
+  const uint32_t b = cell_start[c], e = cell_start[c + 1];
+  for (uint32_t s = b + 1; s < e; ++s) {          // insertion sort, a handful of entries at most
+    const uint32_t v = cell_pid[s];
+    uint32_t t = s;
+    while (t > b && cell_pid[t - 1] > v) { cell_pid[t] = cell_pid[t - 1]; --t; }
+    cell_pid[t] = v;
+  }
+  for (uint32_t s = b; s < e; ++s) {
+    const uint32_t i = cell_pid[s];
+    float4 p = pos[i];
+    p.w = __uint_as_float(i);
+    cpos[s] = p;
+    if (ANISO) {
+      const V3 a = quat_axis(as_q(quat[i]));
+      caxis[s] = make_float4(a.x, a.y, a.z, 0.0f);
+    }
+  }
+}
+
+}  // namespace hpmc

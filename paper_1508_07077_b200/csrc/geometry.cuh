@@ -1,0 +1,189 @@
+// geometry.cuh -- fp32 shape arithmetic of the hot path.  Compiled with --fmad=false: no contraction; an FMA
+// happens only where fmaf() is written (dot3).  Division and square root are IEEE (__fdiv_rn, __fsqrt_rn).
+//   depletant-vs-colloid tests: sphere; point-to-half-ball (R-S16); point-to-disc (R-S17)
+//   colloid-vs-colloid: sphere distance; support-function MPR test for the convex shapes (R-S18)
+//   rotation: Cayley move (R-S6), body axis from the quaternion (R-S19)
+// Paper: the overlap tests realise U_ij = infinity for overlapping pairs in Eq. 5 (L80) and the
+// colloid-depletant overlap of Fig. 2 (L72); the paper gives no algorithm for them (ref. 35).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace hpmc {
+
+enum : int { SH_SPHERE = 0, SH_HALFBALL = 1, SH_SPHERODISK = 2 };
+
+struct Geo {              // derived constants, computed once on the host in fp32
+  float L, halfL, w;      // box edge, L/2, cell width
+  int nc;                 // cells per axis
+  float Rins, Rins2;      // insertion-sphere radius (sigma_c+sigma_d)/2 and square
+  float dcirc2;           // sigma_c^2
+  float rcut2;            // neighbour pre-filter radius squared
+  float rd, rd2;          // depletant radius
+  float Rh, cen;          // half-ball radius and interior-point offset 3 Rh / 8
+  float adisk, sdisk, rs2;
+};
+
+struct V3 { float x, y, z; };
+
+__device__ __forceinline__ V3 v3(float x, float y, float z) { return V3{x, y, z}; }
+__device__ __forceinline__ V3 operator+(V3 a, V3 b) { return V3{a.x + b.x, a.y + b.y, a.z + b.z}; }
+__device__ __forceinline__ V3 operator-(V3 a, V3 b) { return V3{a.x - b.x, a.y - b.y, a.z - b.z}; }
+__device__ __forceinline__ V3 operator*(V3 a, float s) { return V3{a.x * s, a.y * s, a.z * s}; }
+__device__ __forceinline__ V3 neg(V3 a) { return V3{-a.x, -a.y, -a.z}; }
+__device__ __forceinline__ float dot3(V3 a, V3 b) { return fmaf(a.z, b.z, fmaf(a.y, b.y, a.x * b.x)); }
+__device__ __forceinline__ V3 cross3(V3 a, V3 b) {
+  return V3{a.y * b.z - a.z * b.y, a.z * b.x - a.x * b.z, a.x * b.y - a.y * b.x};
+}
+__device__ __forceinline__ bool is_zero(V3 a) { return a.x == 0.0f && a.y == 0.0f && a.z == 0.0f; }
+
+// Quaternion (w,x,y,z); stored in memory as float4 with .x = w, .y = x, .z = y, .w = z.
+struct Q4 { float w, x, y, z; };
+__device__ __forceinline__ Q4 as_q(float4 f) { return Q4{f.x, f.y, f.z, f.w}; }
+__device__ __forceinline__ float4 as_f4(Q4 q) { return make_float4(q.w, q.x, q.y, q.z); }
+
+// body z axis in the space frame: third column of the rotation matrix of q (R-S19)
+__device__ __forceinline__ V3 quat_axis(Q4 q) {
+  return V3{2.0f * (q.x * q.z + q.w * q.y), 2.0f * (q.y * q.z - q.w * q.x), 1.0f - 2.0f * (q.x * q.x + q.y * q.y)};
+}
+
+// Cayley rotation move (R-S6): q' = normalise((1,v) (x) q), multiplication on the left (space frame)
+__device__ __forceinline__ Q4 rotate_cayley(Q4 q, V3 v) {
+  const float pw = q.w - ((v.x * q.x + v.y * q.y) + v.z * q.z);
+  const float px = (q.x + v.x * q.w) + (v.y * q.z - v.z * q.y);
+  const float py = (q.y + v.y * q.w) + (v.z * q.x - v.x * q.z);
+  const float pz = (q.z + v.z * q.w) + (v.x * q.y - v.y * q.x);
+  const float n2 = (pw * pw + px * px) + (py * py + pz * pz);
+  const float n = __fsqrt_rn(n2);
+  return Q4{__fdiv_rn(pw, n), __fdiv_rn(px, n), __fdiv_rn(py, n), __fdiv_rn(pz, n)};
+}
+
+// Does a depletant centred at d (relative to the colloid centre) overlap the colloid with body axis a?
+template <int SHAPE>
+__device__ __forceinline__ bool dep_overlap(const Geo& g, V3 d, V3 a) {
+  const float d2 = dot3(d, d);
+  if (!(d2 < g.Rins2)) return false;
+  if (SHAPE == SH_SPHERE) return true;
+  const float bz = dot3(d, a);
+  if (SHAPE == SH_HALFBALL) {
+    if (bz <= 0.0f) return true;
+    const V3 p = V3{d.x - bz * a.x, d.y - bz * a.y, d.z - bz * a.z};
+    const float rho = __fsqrt_rn(dot3(p, p));
+    if (rho <= g.Rh) return bz < g.rd;
+    const float e = rho - g.Rh;
+    return fmaf(e, e, bz * bz) < g.rd2;
+  }
+  const V3 p = V3{d.x - bz * a.x, d.y - bz * a.y, d.z - bz * a.z};
+  const float rho = __fsqrt_rn(dot3(p, p));
+  if (rho <= g.adisk) return bz * bz < g.rs2;
+  const float e = rho - g.adisk;
+  return fmaf(e, e, bz * bz) < g.rs2;
+}
+
+template <int SHAPE>
+__device__ __forceinline__ V3 support(const Geo& g, V3 a, V3 n) {
+  const float nz = dot3(n, a);
+  if (SHAPE == SH_HALFBALL) {
+    if (nz <= 0.0f) {
+      const float len = __fsqrt_rn(dot3(n, n));
+      if (!(len > 0.0f)) return V3{0.0f, 0.0f, 0.0f};
+      return n * __fdiv_rn(g.Rh, len);
+    }
+    const V3 p = V3{n.x - nz * a.x, n.y - nz * a.y, n.z - nz * a.z};
+    const float l = __fsqrt_rn(dot3(p, p));
+    if (!(l > 0.0f)) return V3{0.0f, 0.0f, 0.0f};
+    return p * __fdiv_rn(g.Rh, l);
+  }
+  const V3 p = V3{n.x - nz * a.x, n.y - nz * a.y, n.z - nz * a.z};
+  const float l = __fsqrt_rn(dot3(p, p));
+  const float len = __fsqrt_rn(dot3(n, n));
+  V3 out = V3{0.0f, 0.0f, 0.0f};
+  if (l > 0.0f) out = p * __fdiv_rn(g.adisk, l);
+  if (len > 0.0f) out = out + n * __fdiv_rn(g.sdisk, len);
+  return out;
+}
+
+template <int SHAPE>
+__device__ __forceinline__ V3 support_diff(const Geo& g, V3 rho, V3 aA, V3 aB, V3 n) {
+  const V3 sb = support<SHAPE>(g, aB, n);
+  const V3 sa = support<SHAPE>(g, aA, neg(n));
+  return (sb + rho) - sa;
+}
+
+#define HPMC_MPR_MAXIT 48
+#define HPMC_MPR_TOL 1e-5f
+
+// Minkowski portal refinement on the full convex shapes: A at the origin (axis aA), B at rho (axis aB).
+template <int SHAPE>
+__device__ __noinline__ bool mpr_overlap(const Geo& g, V3 rho, V3 aA, V3 aB) {
+  V3 cA = V3{0.0f, 0.0f, 0.0f}, cB = rho;
+  if (SHAPE == SH_HALFBALL) {
+    cA = neg(aA * g.cen);
+    cB = rho - aB * g.cen;
+  }
+  V3 v0 = cB - cA;
+  if (is_zero(v0)) v0 = V3{1e-5f, 0.0f, 0.0f};
+  V3 n = neg(v0);
+  V3 v1 = support_diff<SHAPE>(g, rho, aA, aB, n);
+  if (dot3(v1, n) <= 0.0f) return false;
+  n = cross3(v1, v0);
+  if (is_zero(n)) return true;
+  V3 v2 = support_diff<SHAPE>(g, rho, aA, aB, n);
+  if (dot3(v2, n) <= 0.0f) return false;
+  n = cross3(v1 - v0, v2 - v0);
+  if (dot3(n, v0) > 0.0f) { const V3 t = v1; v1 = v2; v2 = t; n = neg(n); }
+  V3 v3;
+  int it = 0;
+  for (;;) {
+    if (it++ >= HPMC_MPR_MAXIT) return true;
+    v3 = support_diff<SHAPE>(g, rho, aA, aB, n);
+    if (dot3(v3, n) <= 0.0f) return false;
+    if (dot3(cross3(v1, v3), v0) < 0.0f) { v2 = v3; n = cross3(v1 - v0, v3 - v0); continue; }
+    if (dot3(cross3(v3, v2), v0) < 0.0f) { v1 = v3; n = cross3(v3 - v0, v2 - v0); continue; }
+    break;
+  }
+  for (it = 0;; ++it) {
+    if (it >= HPMC_MPR_MAXIT) return true;
+    n = cross3(v2 - v1, v3 - v1);
+    const float len = __fsqrt_rn(dot3(n, n));
+    if (!(len > 0.0f)) return true;
+    n = V3{__fdiv_rn(n.x, len), __fdiv_rn(n.y, len), __fdiv_rn(n.z, len)};
+    if (dot3(n, v1) >= 0.0f) return true;
+    const V3 v4 = support_diff<SHAPE>(g, rho, aA, aB, n);
+    if (dot3(v4, n) < 0.0f) return false;
+    if (dot3(v4 - v3, n) <= HPMC_MPR_TOL) return false;
+    const V3 c = cross3(v4, v0);
+    if (dot3(v1, c) > 0.0f) {
+      if (dot3(v2, c) > 0.0f) v1 = v4; else v3 = v4;
+    } else {
+      if (dot3(v3, c) > 0.0f) v2 = v4; else v1 = v4;
+    }
+  }
+}
+
+template <int SHAPE>
+__device__ __forceinline__ bool pair_overlap(const Geo& g, V3 rho, V3 aA, V3 aB) {
+  const float r2 = dot3(rho, rho);
+  if (!(r2 < g.dcirc2)) return false;
+  if (SHAPE == SH_SPHERE) return true;
+  return mpr_overlap<SHAPE>(g, rho, aA, aB);
+}
+
+// periodic helpers (R-S13)
+__device__ __forceinline__ float minimg1(const Geo& g, float d) {
+  if (d > g.halfL) d -= g.L; else if (d < -g.halfL) d += g.L;
+  return d;
+}
+__device__ __forceinline__ float wrap1(const Geo& g, float x) {
+  if (x < 0.0f) x += g.L;
+  if (x >= g.L) x -= g.L;
+  return x;
+}
+__device__ __forceinline__ int cell_axis(const Geo& g, float x, float shift) {
+  float t = x - shift;
+  if (t < 0.0f) t += g.L;
+  int c = (int)__fdiv_rn(t, g.w);
+  if (c >= g.nc) c = g.nc - 1;
+  return c;
+}
+
+}  // namespace hpmc

@@ -1,0 +1,445 @@
+// hpmc_lib.cu -- host driver and C-ABI (include/hpmc.h) of the B200 implicit-depletant HPMC library.
+//
+// Per sweep:
+//   hpmc_build_cells: host draws the grid shift from Philox(seed, step, SWEEP) -> K-A kernels (cells.cuh)
+//   hpmc_sweep:       host draws the colour permutation, builds/caches the Poisson threshold table (fp64, R-S2)
+//                     -> 8 launches of the move kernel (move.cuh), one per sub-lattice, stream ordered.
+// No host synchronisation inside a sweep; no CPU fallback anywhere.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/hpmc.h"
+#include "cells.cuh"
+#include "move.cuh"
+
+using namespace hpmc;
+
+namespace {
+
+thread_local std::string g_init_error;
+
+struct PoissonTable {
+  double lambda = -1.0;
+  uint32_t k_lo = 0;
+  int n = 0;
+  unsigned long long* d_T = nullptr;
+  size_t cap = 0;
+};
+
+struct EventPair { cudaEvent_t a, b; };
+
+}  // namespace
+
+struct hpmc_ctx {
+  hpmc_params p;
+  Geo g;
+  int64_t N = 0;
+  int ncell = 0;
+  cudaStream_t stream = nullptr;
+  bool own_pose = false;
+  float4* d_pos = nullptr;
+  float4* d_quat = nullptr;
+  float4* d_cpos = nullptr;
+  float4* d_caxis = nullptr;
+  uint32_t *d_cid = nullptr, *d_rank = nullptr, *d_counts = nullptr, *d_cell_start = nullptr, *d_cell_pid = nullptr,
+           *d_tile_sums = nullptr;
+  int ntiles = 0;
+  uint8_t* d_outcome = nullptr;
+  unsigned long long* d_counters = nullptr;
+  int* d_err = nullptr;
+  float shift[3] = {0, 0, 0};
+  bool built = false;
+  uint32_t b_seed = 0, b_step = 0;
+  std::vector<PoissonTable> tables;     // small cache keyed by lambda (C2 sweeps four densities)
+  size_t table_rr = 0;
+  int num_sms = 148;
+  int move_ctas = 0;
+  int64_t launches = 0;
+  bool timing = false;
+  std::vector<EventPair> ev;
+  size_t ev_used = 0;
+  double ev_ms = 0.0;
+  int64_t ev_launches = 0;
+  std::string err;
+};
+
+namespace {
+
+int fail(hpmc_ctx* c, int code, const std::string& msg) {
+  if (c) c->err = msg; else g_init_error = msg;
+  return code;
+}
+
+#define CU(call)                                                                                   \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess)                                                                         \
+      return fail(ctx, HPMC_E_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_));           \
+  } while (0)
+
+Geo make_geo(const hpmc_params& p, int nc) {
+  Geo g;
+  g.L = p.box_L; g.halfL = 0.5f * p.box_L; g.nc = nc; g.w = p.box_L / (float)nc;
+  g.rd = 0.5f * p.sigma_d;
+  g.Rins = 0.5f * (p.sigma_c + p.sigma_d);
+  g.Rins2 = g.Rins * g.Rins;
+  g.dcirc2 = p.sigma_c * p.sigma_c;
+  const float rcut = ((p.sigma_c + p.sigma_d) + p.d_max_cap * 1.7320508f) + 1e-3f;
+  g.rcut2 = rcut * rcut;
+  g.Rh = 0.5f * p.sigma_c;
+  g.cen = 0.375f * g.Rh;
+  g.adisk = p.disk_a; g.sdisk = p.disk_s;
+  const float rs = p.disk_s + g.rd;
+  g.rs2 = rs * rs;
+  g.rd2 = g.rd * g.rd;
+  return g;
+}
+
+// Poisson thresholds T[j] = floor(CDF(k_lo + j) 2^64), saturating (R-S2); fp64 on the host.
+void poisson_thresholds(double lambda, uint32_t& k_lo, std::vector<unsigned long long>& T) {
+  T.clear(); k_lo = 0;
+  if (!(lambda > 0.0)) return;
+  const double sq = std::sqrt(lambda);
+  long long lo = (long long)std::floor(lambda - 10.0 * sq - 10.0);
+  if (lo < 0) lo = 0;
+  const long long hi = (long long)std::ceil(lambda + 10.0 * sq + 20.0);
+  const long long n = hi - lo + 1;
+  long long m = (long long)std::floor(lambda);
+  if (m < lo) m = lo;
+  std::vector<double> pm((size_t)n);
+  pm[(size_t)(m - lo)] = std::exp((double)m * std::log(lambda) - lambda - std::lgamma((double)m + 1.0));
+  for (long long k = m; k < hi; ++k) pm[(size_t)(k + 1 - lo)] = pm[(size_t)(k - lo)] * lambda / (double)(k + 1);
+  for (long long k = m; k > lo; --k) pm[(size_t)(k - 1 - lo)] = pm[(size_t)(k - lo)] * (double)k / lambda;
+  double S = 0.0;
+  for (long long j = 0; j < n; ++j) S += pm[(size_t)j];
+  k_lo = (uint32_t)lo;
+  T.resize((size_t)n);
+  double c = 0.0;
+  for (long long j = 0; j < n; ++j) {
+    c += pm[(size_t)j] / S;
+    T[(size_t)j] = (c >= 1.0) ? 0xFFFFFFFFFFFFFFFFull : (unsigned long long)std::floor(c * 18446744073709551616.0);
+  }
+}
+
+int get_table(hpmc_ctx* ctx, double lambda, PoissonTable** out) {
+  for (auto& t : ctx->tables)
+    if (t.lambda == lambda) { *out = &t; return 0; }
+  PoissonTable* slot;
+  if (ctx->tables.size() < 8) { ctx->tables.emplace_back(); slot = &ctx->tables.back(); }
+  else {
+    // evicting a table that may still be read by queued kernels: drain the stream first
+    CU(cudaStreamSynchronize(ctx->stream));
+    slot = &ctx->tables[ctx->table_rr++ % ctx->tables.size()];
+  }
+  std::vector<unsigned long long> T;
+  uint32_t klo;
+  poisson_thresholds(lambda, klo, T);
+  if (T.size() > slot->cap) {
+    if (slot->d_T) { CU(cudaStreamSynchronize(ctx->stream)); CU(cudaFree(slot->d_T)); slot->d_T = nullptr; }
+    slot->cap = T.size() + 64;
+    CU(cudaMalloc(&slot->d_T, slot->cap * sizeof(unsigned long long)));
+  }
+  if (!T.empty()) {
+    // pageable source: the runtime stages it before returning, so T may go out of scope
+    CU(cudaMemcpyAsync(slot->d_T, T.data(), T.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+  }
+  slot->lambda = lambda; slot->k_lo = klo; slot->n = (int)T.size();
+  *out = slot;
+  return 0;
+}
+
+template <int SHAPE>
+int launch_move(hpmc_ctx* ctx, const MoveArgs& a, bool cb) {
+  const dim3 grid(ctx->move_ctas), block(MOVE_WARPS * 32);
+  if (cb) k_move<SHAPE, true><<<grid, block, 0, ctx->stream>>>(a);
+  else k_move<SHAPE, false><<<grid, block, 0, ctx->stream>>>(a);
+  return 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+int hpmc_init(hpmc_ctx** out, const hpmc_params* p, int64_t N, float* d_pos4, float* d_quat4, void* cuda_stream) {
+  hpmc_ctx* ctx = nullptr;
+  if (!out || !p) return fail(nullptr, HPMC_E_BADARG, "hpmc_init: NULL argument");
+  *out = nullptr;
+  if (N <= 0 || N > 0x7fffffff) return fail(nullptr, HPMC_E_BADARG, "hpmc_init: N out of range");
+  if (!(p->box_L > 0.0f) || !(p->sigma_c > 0.0f) || p->sigma_d < 0.0f || p->d_max_cap < 0.0f)
+    return fail(nullptr, HPMC_E_BADARG, "hpmc_init: bad geometry parameters");
+  if (p->shape < HPMC_SPHERE || p->shape > HPMC_SPHERODISK) return fail(nullptr, HPMC_E_BADARG, "hpmc_init: bad shape");
+  if (p->shape != HPMC_SPHERE && d_pos4 && !d_quat4)
+    return fail(nullptr, HPMC_E_BADARG, "hpmc_init: anisotropic shape needs orientations");
+  if (!d_pos4 && d_quat4) return fail(nullptr, HPMC_E_BADARG, "hpmc_init: d_quat4 without d_pos4");
+  const double wmin = (double)p->sigma_c + (double)p->sigma_d + 2.0 * (double)p->d_max_cap;
+  long long n = (long long)std::floor((double)p->box_L / wmin);
+  n &= ~1ll;
+  if (n < 4) return fail(nullptr, HPMC_E_GEOMETRY, "hpmc_init: fewer than 4 cells per axis");
+  if (n > 1024) return fail(nullptr, HPMC_E_GEOMETRY, "hpmc_init: more than 1024 cells per axis");
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+    return fail(nullptr, HPMC_E_CUDA, std::string("hpmc_init: no usable CUDA device: ") + cudaGetErrorString(cudaGetLastError()));
+
+  ctx = new hpmc_ctx();
+  ctx->p = *p; ctx->N = N; ctx->stream = (cudaStream_t)cuda_stream; ctx->num_sms = sms;
+  ctx->g = make_geo(*p, (int)n);
+  ctx->ncell = (int)(n * n * n);
+  ctx->ntiles = (ctx->ncell + SCAN_TILE - 1) / SCAN_TILE;
+  auto bail = [&](const std::string& m) { g_init_error = m; hpmc_destroy(ctx); return HPMC_E_CUDA; };
+#define CUI(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return bail(std::string(#call) + ": " + cudaGetErrorString(e_)); } while (0)
+  if (!d_pos4) {
+    ctx->own_pose = true;
+    CUI(cudaMalloc(&ctx->d_pos, sizeof(float4) * N));
+    CUI(cudaMalloc(&ctx->d_quat, sizeof(float4) * N));
+    CUI(cudaMemsetAsync(ctx->d_pos, 0, sizeof(float4) * N, ctx->stream));
+    CUI(cudaMemsetAsync(ctx->d_quat, 0, sizeof(float4) * N, ctx->stream));
+  } else {
+    ctx->d_pos = (float4*)d_pos4; ctx->d_quat = (float4*)d_quat4;
+  }
+  CUI(cudaMalloc(&ctx->d_cpos, sizeof(float4) * N));
+  if (p->shape != HPMC_SPHERE) CUI(cudaMalloc(&ctx->d_caxis, sizeof(float4) * N));
+  CUI(cudaMalloc(&ctx->d_cid, sizeof(uint32_t) * N));
+  CUI(cudaMalloc(&ctx->d_rank, sizeof(uint32_t) * N));
+  CUI(cudaMalloc(&ctx->d_cell_pid, sizeof(uint32_t) * N));
+  CUI(cudaMalloc(&ctx->d_counts, sizeof(uint32_t) * ctx->ncell));
+  CUI(cudaMalloc(&ctx->d_cell_start, sizeof(uint32_t) * ((size_t)ctx->ncell + 1)));
+  CUI(cudaMalloc(&ctx->d_tile_sums, sizeof(uint32_t) * (size_t)ctx->ntiles));
+  CUI(cudaMalloc(&ctx->d_outcome, (size_t)N));
+  CUI(cudaMalloc(&ctx->d_counters, sizeof(unsigned long long) * C_COUNT));
+  CUI(cudaMalloc(&ctx->d_err, sizeof(int)));
+  CUI(cudaMemsetAsync(ctx->d_outcome, 0, (size_t)N, ctx->stream));
+  CUI(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * C_COUNT, ctx->stream));
+  CUI(cudaMemsetAsync(ctx->d_err, 0, sizeof(int), ctx->stream));
+#undef CUI
+  // persistent warps: a whole number of CTAs per SM, capped by the work available
+  const int nact = ctx->ncell / 8;
+  int ctas = sms * 8;
+  const int need = (nact + MOVE_WARPS - 1) / MOVE_WARPS;
+  if (ctas > need) ctas = need;
+  if (ctas < 1) ctas = 1;
+  ctx->move_ctas = ctas;
+  *out = ctx;
+  return HPMC_OK;
+}
+
+void hpmc_destroy(hpmc_ctx* ctx) {
+  if (!ctx) return;
+  cudaStreamSynchronize(ctx->stream);
+  if (ctx->own_pose) { cudaFree(ctx->d_pos); cudaFree(ctx->d_quat); }
+  cudaFree(ctx->d_cpos); cudaFree(ctx->d_caxis); cudaFree(ctx->d_cid); cudaFree(ctx->d_rank);
+  cudaFree(ctx->d_cell_pid); cudaFree(ctx->d_counts); cudaFree(ctx->d_cell_start); cudaFree(ctx->d_tile_sums);
+  cudaFree(ctx->d_outcome); cudaFree(ctx->d_counters); cudaFree(ctx->d_err);
+  for (auto& t : ctx->tables) cudaFree(t.d_T);
+  for (auto& e : ctx->ev) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+  delete ctx;
+}
+
+int hpmc_build_cells(hpmc_ctx* ctx, uint32_t seed, uint32_t step) {
+  if (!ctx) return HPMC_E_BADARG;
+  const Key10 key = make_key(seed, step);
+  const Block4 r = philox(key, 0, 0, 0, ctr_word3(P_SWEEP, 0, 0));
+  ctx->shift[0] = unit01(r.x) * ctx->g.w;
+  ctx->shift[1] = unit01(r.y) * ctx->g.w;
+  ctx->shift[2] = unit01(r.z) * ctx->g.w;
+  const int N = (int)ctx->N, nb = (N + 255) / 256;
+  cudaStream_t st = ctx->stream;
+  CU(cudaMemsetAsync(ctx->d_counts, 0, sizeof(uint32_t) * ctx->ncell, st));
+  k_bin_count<<<nb, 256, 0, st>>>(ctx->d_pos, N, ctx->g, ctx->shift[0], ctx->shift[1], ctx->shift[2], ctx->d_cid,
+                                  ctx->d_rank, ctx->d_counts);
+  k_scan_tiles<<<ctx->ntiles, SCAN_THREADS, 0, st>>>(ctx->d_counts, ctx->ncell, ctx->d_tile_sums);
+  k_scan_top<<<1, 1024, 0, st>>>(ctx->d_tile_sums, ctx->ntiles);
+  k_scan_apply<<<ctx->ntiles, SCAN_THREADS, 0, st>>>(ctx->d_counts, ctx->ncell, ctx->d_tile_sums, ctx->d_cell_start);
+  k_fill<<<nb, 256, 0, st>>>(ctx->d_cid, ctx->d_rank, ctx->d_cell_start, N, ctx->d_cell_pid);
+  const int cbk = (ctx->ncell + 255) / 256;
+  if (ctx->p.shape == HPMC_SPHERE)
+    k_sort_write<false><<<cbk, 256, 0, st>>>(ctx->d_cell_start, ctx->ncell, ctx->d_cell_pid, ctx->d_pos, ctx->d_quat,
+                                             ctx->d_cpos, ctx->d_caxis);
+  else
+    k_sort_write<true><<<cbk, 256, 0, st>>>(ctx->d_cell_start, ctx->ncell, ctx->d_cell_pid, ctx->d_pos, ctx->d_quat,
+                                            ctx->d_cpos, ctx->d_caxis);
+  ctx->launches += 6;
+  CU(cudaGetLastError());
+  ctx->built = true; ctx->b_seed = seed; ctx->b_step = step;
+  return HPMC_OK;
+}
+
+int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_max, float a_max, int32_t n_trial) {
+  if (!ctx) return HPMC_E_BADARG;
+  if (!(d_max >= 0.0f) || !(n_R >= 0.0) || !(a_max >= 0.0f) || n_trial < 0 || n_trial > 65535)
+    return fail(ctx, HPMC_E_BADARG, "hpmc_sweep: bad argument");
+  if (d_max > ctx->p.d_max_cap) return fail(ctx, HPMC_E_DMAX, "hpmc_sweep: d_max exceeds d_max_cap");
+  if (!ctx->built || ctx->b_seed != seed || ctx->b_step != step)
+    return fail(ctx, HPMC_E_STATE, "hpmc_sweep: call hpmc_build_cells(seed, step) first");
+  const double Rd = (double)ctx->g.Rins;
+  const double lambda = n_R * ((4.0 * M_PI / 3.0) * (Rd * Rd * Rd));
+  PoissonTable* pt = nullptr;
+  const int rc = get_table(ctx, lambda, &pt);
+  if (rc) return rc;
+
+  const Key10 key = make_key(seed, step);
+  // colour permutation (R-2): Fisher-Yates from SWEEP blocks 1 and 2
+  uint32_t perm[8] = {0, 1, 2, 3, 4, 5, 6, 7};
+  const Block4 b1 = philox(key, 0, 0, 0, ctr_word3(P_SWEEP, 0, 1));
+  const Block4 b2 = philox(key, 0, 0, 0, ctr_word3(P_SWEEP, 0, 2));
+  const uint32_t wds[7] = {b1.x, b1.y, b1.z, b1.w, b2.x, b2.y, b2.z};
+  for (int i = 7, j = 0; i >= 1; --i, ++j) {
+    const uint32_t r = (uint32_t)(((uint64_t)wds[j] * (uint32_t)(i + 1)) >> 32);
+    const uint32_t t = perm[i]; perm[i] = perm[r]; perm[r] = t;
+  }
+  CU(cudaMemsetAsync(ctx->d_outcome, 0, (size_t)ctx->N, ctx->stream));
+
+  MoveArgs a;
+  a.g = ctx->g; a.key = key;
+  a.sx = ctx->shift[0]; a.sy = ctx->shift[1]; a.sz = ctx->shift[2];
+  a.hc = ctx->g.nc / 2; a.nact = a.hc * a.hc * a.hc;
+  a.d_max = d_max; a.a_max = a_max; a.a_max2 = a_max * a_max; a.n_trial = n_trial;
+  a.pos = ctx->d_pos; a.quat = ctx->d_quat; a.cpos = ctx->d_cpos; a.caxis = ctx->d_caxis;
+  a.cell_start = ctx->d_cell_start;
+  a.ptable = pt->d_T; a.pt_n = pt->n; a.pt_klo = pt->k_lo;
+  a.outcome = ctx->d_outcome; a.counters = ctx->d_counters; a.err_flag = ctx->d_err;
+  const bool cb = n_trial > 0;
+  for (int pass = 0; pass < 8; ++pass) {
+    a.colour = perm[pass];
+    EventPair* ep = nullptr;
+    if (ctx->timing) {
+      if (ctx->ev_used == ctx->ev.size()) {
+        EventPair e;
+        CU(cudaEventCreate(&e.a)); CU(cudaEventCreate(&e.b));
+        ctx->ev.push_back(e);
+      }
+      ep = &ctx->ev[ctx->ev_used++];
+      CU(cudaEventRecord(ep->a, ctx->stream));
+    }
+    switch (ctx->p.shape) {
+      case HPMC_SPHERE: launch_move<SH_SPHERE>(ctx, a, cb); break;
+      case HPMC_HALFBALL: launch_move<SH_HALFBALL>(ctx, a, cb); break;
+      default: launch_move<SH_SPHERODISK>(ctx, a, cb); break;
+    }
+    if (ep) CU(cudaEventRecord(ep->b, ctx->stream));
+  }
+  ctx->launches += 8;
+  CU(cudaGetLastError());
+  ctx->built = false;
+  return HPMC_OK;
+}
+
+int hpmc_run(hpmc_ctx* ctx, uint32_t seed, uint32_t step0, int64_t n_sweeps, double n_R, float d_max, float a_max,
+             int32_t n_trial) {
+  for (int64_t s = 0; s < n_sweeps; ++s) {
+    int rc = hpmc_build_cells(ctx, seed, step0 + (uint32_t)s);
+    if (rc) return rc;
+    rc = hpmc_sweep(ctx, seed, step0 + (uint32_t)s, n_R, d_max, a_max, n_trial);
+    if (rc) return rc;
+  }
+  return HPMC_OK;
+}
+
+static int check_err_flag(hpmc_ctx* ctx) {
+  int e = 0;
+  CU(cudaMemcpyAsync(&e, ctx->d_err, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  if (e) return fail(ctx, HPMC_E_NEIGHBOR_OVERFLOW, "move kernel: more than MAXNB neighbours in range");
+  return HPMC_OK;
+}
+
+int hpmc_counters(hpmc_ctx* ctx, hpmc_counters_t* host_out) {
+  if (!ctx || !host_out) return HPMC_E_BADARG;
+  static_assert(sizeof(hpmc_counters_t) == sizeof(unsigned long long) * C_COUNT, "counter layout");
+  CU(cudaMemcpyAsync(host_out, ctx->d_counters, sizeof(hpmc_counters_t), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  return check_err_flag(ctx);
+}
+
+int hpmc_reset_counters(hpmc_ctx* ctx) {
+  if (!ctx) return HPMC_E_BADARG;
+  CU(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * C_COUNT, ctx->stream));
+  return HPMC_OK;
+}
+
+int hpmc_outcomes(hpmc_ctx* ctx, uint8_t* d_outcome) {
+  if (!ctx || !d_outcome) return HPMC_E_BADARG;
+  CU(cudaMemcpyAsync(d_outcome, ctx->d_outcome, (size_t)ctx->N, cudaMemcpyDeviceToDevice, ctx->stream));
+  return HPMC_OK;
+}
+
+int hpmc_grid(hpmc_ctx* ctx, int32_t* n_c, float* w) {
+  if (!ctx || !n_c || !w) return HPMC_E_BADARG;
+  *n_c = ctx->g.nc; *w = ctx->g.w;
+  return HPMC_OK;
+}
+
+int hpmc_cells(hpmc_ctx* ctx, uint32_t* d_cell_start, uint32_t* d_cell_pid, float* host_shift3) {
+  if (!ctx || !d_cell_start || !d_cell_pid || !host_shift3) return HPMC_E_BADARG;
+  CU(cudaMemcpyAsync(d_cell_start, ctx->d_cell_start, sizeof(uint32_t) * ((size_t)ctx->ncell + 1),
+                     cudaMemcpyDeviceToDevice, ctx->stream));
+  CU(cudaMemcpyAsync(d_cell_pid, ctx->d_cell_pid, sizeof(uint32_t) * (size_t)ctx->N, cudaMemcpyDeviceToDevice,
+                     ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  for (int a = 0; a < 3; ++a) host_shift3[a] = ctx->shift[a];
+  return HPMC_OK;
+}
+
+int hpmc_upload(hpmc_ctx* ctx, const float* host_pos4, const float* host_quat4) {
+  if (!ctx || !host_pos4) return HPMC_E_BADARG;
+  CU(cudaMemcpyAsync(ctx->d_pos, host_pos4, sizeof(float4) * ctx->N, cudaMemcpyHostToDevice, ctx->stream));
+  if (host_quat4 && ctx->d_quat)
+    CU(cudaMemcpyAsync(ctx->d_quat, host_quat4, sizeof(float4) * ctx->N, cudaMemcpyHostToDevice, ctx->stream));
+  return HPMC_OK;
+}
+
+int hpmc_download(hpmc_ctx* ctx, float* host_pos4, float* host_quat4, uint8_t* host_outcome) {
+  if (!ctx) return HPMC_E_BADARG;
+  if (host_pos4) CU(cudaMemcpyAsync(host_pos4, ctx->d_pos, sizeof(float4) * ctx->N, cudaMemcpyDeviceToHost, ctx->stream));
+  if (host_quat4 && ctx->d_quat)
+    CU(cudaMemcpyAsync(host_quat4, ctx->d_quat, sizeof(float4) * ctx->N, cudaMemcpyDeviceToHost, ctx->stream));
+  if (host_outcome) CU(cudaMemcpyAsync(host_outcome, ctx->d_outcome, (size_t)ctx->N, cudaMemcpyDeviceToHost, ctx->stream));
+  return HPMC_OK;
+}
+
+int hpmc_step_host(hpmc_ctx* ctx, float* host_pos4, float* host_quat4, uint8_t* host_outcome, uint32_t seed,
+                   uint32_t step, double n_R, float d_max, float a_max, int32_t n_trial) {
+  int rc = hpmc_upload(ctx, host_pos4, host_quat4);
+  if (rc) return rc;
+  rc = hpmc_build_cells(ctx, seed, step);
+  if (rc) return rc;
+  rc = hpmc_sweep(ctx, seed, step, n_R, d_max, a_max, n_trial);
+  if (rc) return rc;
+  rc = hpmc_download(ctx, host_pos4, host_quat4, host_outcome);
+  if (rc) return rc;
+  return check_err_flag(ctx);
+}
+
+int64_t hpmc_launch_count(hpmc_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int hpmc_time_move_kernel(hpmc_ctx* ctx, int32_t enable) {
+  if (!ctx) return HPMC_E_BADARG;
+  CU(cudaStreamSynchronize(ctx->stream));
+  ctx->timing = enable != 0;
+  ctx->ev_used = 0; ctx->ev_ms = 0.0; ctx->ev_launches = 0;
+  return HPMC_OK;
+}
+
+int hpmc_move_kernel_ms(hpmc_ctx* ctx, double* ms_total, int64_t* launches) {
+  if (!ctx || !ms_total || !launches) return HPMC_E_BADARG;
+  CU(cudaStreamSynchronize(ctx->stream));
+  for (size_t i = 0; i < ctx->ev_used; ++i) {
+    float ms = 0.0f;
+    CU(cudaEventElapsedTime(&ms, ctx->ev[i].a, ctx->ev[i].b));
+    ctx->ev_ms += ms;
+  }
+  ctx->ev_launches += (int64_t)ctx->ev_used;
+  ctx->ev_used = 0;
+  *ms_total = ctx->ev_ms; *launches = ctx->ev_launches;
+  return HPMC_OK;
+}
+
+const char* hpmc_last_error(hpmc_ctx* ctx) { return ctx ? ctx->err.c_str() : g_init_error.c_str(); }
+
+}  // extern "C"

@@ -1,0 +1,210 @@
+"""GPU parity: the CUDA path (through the C-ABI, include/hpmc.h) against the CPU oracle, element by element,
+on the same seeded inputs.  Bar (BASELINE.json north_star): per-move outcome codes and fp32 poses BIT-EXACT
+after every sweep; integer counters that both sides define (everything except dep_evaluated / philox_blocks,
+which describe each implementation's own work) equal.
+
+Default sweep counts keep the suite to a few minutes; HPMC_PARITY_FULL=1 runs the configs' full lengths
+(min(1000, sweeps) per north_star).
+"""
+import os
+
+import numpy as np
+import pytest
+
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+FULL = os.environ.get("HPMC_PARITY_FULL", "0") == "1"
+SHARED_COUNTERS = ("trials_trans", "accept_trans", "trials_rot", "accept_rot", "rej_boundary", "rej_hard",
+                   "rej_depletant", "rej_cb", "dep_drawn", "dep_needed", "cb_reinsertions")
+
+
+def _mk(cfg, pos, quat, threads=None):
+    import torch
+    import oracle
+    import paper_1508_07077_b200 as hp
+    o = oracle.Oracle(cfg.shape, cfg.sigma_c, cfg.sigma_d, cfg.box_L, cfg.d_max, pos, quat, cfg.disk_a, cfg.disk_s,
+                      threads=threads or os.cpu_count())
+    dpos = torch.from_numpy(pos.copy()).cuda()
+    dquat = None if quat is None else torch.from_numpy(quat.copy()).cuda()
+    h = hp.HPMC(cfg.shape, cfg.sigma_c, cfg.sigma_d, cfg.box_L, cfg.d_max, dpos, dquat, cfg.disk_a, cfg.disk_s)
+    return o, h, dpos, dquat
+
+
+def _bits(a):
+    return np.ascontiguousarray(a).view(np.uint32)
+
+
+def run_parity(cfg, pos, quat, sweeps, n_R, step0=0, check_cells_every=10):
+    o, h, dpos, dquat = _mk(cfg, pos, quat)
+    assert (o.n_c, np.float32(o.w)) == (h.n_c, np.float32(h.w))
+    for s in range(step0, step0 + sweeps):
+        o.build_cells(cfg.seed, s)
+        h.build_cells(cfg.seed, s)
+        if (s - step0) % check_cells_every == 0:
+            cs, cp, sh = h.cells()
+            ocs, ocp, osh = o.cells()
+            assert np.array_equal(np.float32(sh), osh)
+            assert np.array_equal(cs.cpu().numpy().view(np.uint32), ocs), "cell_start differs at sweep %d" % s
+            assert np.array_equal(cp.cpu().numpy().view(np.uint32), ocp), "cell_pid differs at sweep %d" % s
+        o.sweep(cfg.seed, s, n_R, cfg.d_max, cfg.a_max, cfg.n_trial)
+        h.sweep(cfg.seed, s, n_R, cfg.d_max, cfg.a_max, cfg.n_trial)
+        out = h.outcomes().cpu().numpy()
+        oo = o.outcomes()
+        if not np.array_equal(out, oo):
+            bad = np.nonzero(out != oo)[0]
+            raise AssertionError("outcome mask differs at sweep %d: %d particles, first %d gpu=%d oracle=%d"
+                                 % (s, len(bad), bad[0], out[bad[0]], oo[bad[0]]))
+        assert np.array_equal(_bits(dpos.cpu().numpy()), _bits(o.pos)), "positions differ at sweep %d" % s
+        if quat is not None:
+            assert np.array_equal(_bits(dquat.cpu().numpy()), _bits(o.quat)), "orientations differ at sweep %d" % s
+    gc, oc = h.counters(), o.counters()
+    for k in SHARED_COUNTERS:
+        assert gc[k] == oc[k], (k, gc[k], oc[k])
+    assert gc["dep_evaluated"] >= gc["dep_needed"]
+    tried = gc["trials_trans"] + gc["trials_rot"]
+    assert tried > 0
+    h.close()
+    return gc
+
+
+def test_c1_spheres_256():
+    cfg = workloads.config("C1")
+    pos, quat = workloads.generate(cfg)
+    c = run_parity(cfg, pos, quat, 100, cfg.n_R(), check_cells_every=1)
+    assert c["accept_trans"] > 0 and c["rej_depletant"] > 0 and c["rej_hard"] > 0 and c["rej_boundary"] > 0
+
+
+def test_c2_spheres_65536_melted_density_sweep():
+    """configs[1]: fcc lattice melted 1000 sweeps (by the ORACLE, n_R = 0), then the four reservoir densities."""
+    import oracle
+    cfg = workloads.config("C2")
+    pos, _ = workloads.generate(cfg)
+    melt = oracle.Oracle(cfg.shape, cfg.sigma_c, cfg.sigma_d, cfg.box_L, cfg.d_max, pos, threads=os.cpu_count())
+    melt.run(cfg.seed, 100000, 1000, 0.0, cfg.d_max)
+    assert melt.counters()["rej_hard"] > 0
+    pos = melt.pos.copy()
+    n = 1000 if FULL else 25
+    for phi in cfg.phi_d_r:
+        run_parity(cfg, pos, None, n, cfg.n_R(phi))
+
+
+def test_c3_spheres_reduced_many_sweeps():
+    cfg = workloads.config("C3", 32768)
+    pos, _ = workloads.generate(cfg)
+    run_parity(cfg, pos, None, 200 if FULL else 40, cfg.n_R())
+
+
+def test_c3_spheres_full_size():
+    """configs[2] at full size (1,048,576 spheres, 1,404,928 cells), the launch configuration bench.py times."""
+    cfg = workloads.config("C3")
+    pos, _ = workloads.generate(cfg)
+    c = run_parity(cfg, pos, None, 200 if FULL else 3, cfg.n_R(), check_cells_every=1)
+    assert c["dep_drawn"] > 2000 * (c["trials_trans"] - c["rej_boundary"] - c["rej_hard"])
+
+
+def test_c3_small_steps_accepting_moves_use_all_depletants():
+    """Accepted moves at C3's density must test all ~2.8k depletants: tiny steps make acceptance common."""
+    import dataclasses
+    cfg = dataclasses.replace(workloads.config("C3", 8192), d_max=0.0005)
+    pos, _ = workloads.generate(cfg)
+    # cell width is fixed by d_max_cap = cfg.d_max here
+    c = run_parity(cfg, pos, None, 10, cfg.n_R())
+    assert c["accept_trans"] > 0.1 * c["trials_trans"]
+
+
+def test_c4_halfballs():
+    cfg = workloads.config("C4")
+    pos, quat = workloads.generate(cfg)
+    c = run_parity(cfg, pos, quat, 500 if FULL else 30, cfg.n_R())
+    assert c["accept_rot"] > 0 and c["accept_trans"] > 0 and c["rej_hard"] > 0
+
+
+def test_c5_spherodisks_configurational_bias():
+    cfg = workloads.config("C5")
+    pos, quat = workloads.generate(cfg)
+    c = run_parity(cfg, pos, quat, 500 if FULL else 30, cfg.n_R())
+    assert c["cb_reinsertions"] > 0 and c["rej_cb"] > 0 and c["accept_rot"] > 0
+
+
+def test_c5_dense_after_compression_hard_overlaps():
+    """More hard-overlap (MPR) decisions: the same discoids in a box 8 % smaller per axis than a loose lattice."""
+    import dataclasses
+    cfg = dataclasses.replace(workloads.config("C5", 4096), phi_c=0.17, n_trial=2)
+    pos, quat = workloads.generate(cfg)
+    c = run_parity(cfg, pos, quat, 60, cfg.n_R())
+    assert c["rej_hard"] > 100
+
+
+@pytest.mark.parametrize("shape", ["sphere", "halfball"])
+def test_edge_cases(shape):
+    import dataclasses
+    base = workloads.config("C1" if shape == "sphere" else "C4", 64 if shape == "halfball" else 48)
+    pos, quat = workloads.generate(base)
+    # (a) no depletants: plain hard-particle MC
+    run_parity(base, pos, quat, 10, 0.0)
+    # (b) zero step: every trial is the identity and is accepted
+    cfg0 = dataclasses.replace(base, d_max=0.0, a_max=0.0)
+    o, h, dpos, dquat = _mk(dataclasses.replace(cfg0, d_max=0.1), pos, quat)
+    o.build_cells(1, 0); h.build_cells(1, 0)
+    o.sweep(1, 0, base.n_R(), 0.0, 0.0, 0); h.sweep(1, 0, base.n_R(), 0.0, 0.0, 0)
+    out = h.outcomes().cpu().numpy()
+    assert np.array_equal(out, o.outcomes()) and set(np.unique(out)) <= {0, 1}
+    h.close()
+    # (c) a single particle (all but one cell empty), CB with the largest trial count the key layout allows
+    one = dataclasses.replace(base, N=1, n_trial=300, phi_c=base.phi_c / base.N)      # same box, one particle
+    p1 = pos[:1].copy()
+    q1 = None if quat is None else quat[:1].copy()
+    o, h, dpos, dquat = _mk(one, p1, q1)
+    for s in range(20):
+        o.build_cells(1, s); h.build_cells(1, s)
+        o.sweep(1, s, base.n_R(), one.d_max, one.a_max, 300); h.sweep(1, s, base.n_R(), one.d_max, one.a_max, 300)
+        assert np.array_equal(h.outcomes().cpu().numpy(), o.outcomes())
+        assert np.array_equal(_bits(dpos.cpu().numpy()), _bits(o.pos))
+    h.close()
+
+
+def test_error_codes():
+    import torch
+    import paper_1508_07077_b200 as hp
+    pos = torch.zeros((8, 4), device="cuda")
+    with pytest.raises(hp.HPMCError) as e:
+        hp.HPMC("sphere", 1.0, 0.2, 3.0, 0.1, pos)             # box too small: n_c < 4
+    assert e.value.code == -2
+    with pytest.raises(hp.HPMCError) as e:
+        hp.HPMC("halfball", 1.0, 0.2, 30.0, 0.1, pos, None)    # anisotropic without orientations
+    assert e.value.code == -1
+    h = hp.HPMC("sphere", 1.0, 0.2, 8.0, 0.1, pos)
+    with pytest.raises(hp.HPMCError) as e:
+        h.sweep(1, 0, 1.0, 0.1)                                 # no build_cells
+    assert e.value.code == -3
+    h.build_cells(1, 0)
+    with pytest.raises(hp.HPMCError) as e:
+        h.sweep(1, 1, 1.0, 0.1)                                 # build for another step
+    assert e.value.code == -3
+    with pytest.raises(hp.HPMCError) as e:
+        h.sweep(1, 0, 1.0, 0.2)                                 # d_max > cap
+    assert e.value.code == -4
+    with pytest.raises(hp.HPMCError) as e:
+        h.sweep(1, 0, -1.0, 0.1)
+    assert e.value.code == -1
+    h.close()
+
+
+def test_host_buffer_step_matches_device_path():
+    """hpmc_step_host (library-owned buffers, host<->device copies inside) gives the same bits."""
+    import torch
+    import paper_1508_07077_b200 as hp
+    cfg = workloads.config("C1")
+    pos, _ = workloads.generate(cfg)
+    o, h, dpos, _ = _mk(cfg, pos, None)
+    hh = hp.HPMC(cfg.shape, cfg.sigma_c, cfg.sigma_d, cfg.box_L, cfg.d_max, None, None, N=cfg.N)
+    hpos = torch.from_numpy(pos.copy()).pin_memory()
+    hout = torch.zeros(cfg.N, dtype=torch.uint8).pin_memory()
+    for s in range(5):
+        o.build_cells(1, s); o.sweep(1, s, cfg.n_R(), cfg.d_max)
+        hh.step_host(hpos, None, hout, 1, s, cfg.n_R(), cfg.d_max)
+        assert np.array_equal(hout.numpy(), o.outcomes())
+        assert np.array_equal(_bits(hpos.numpy()), _bits(o.pos))
+    hh.close(); h.close()
