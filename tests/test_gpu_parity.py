@@ -140,7 +140,7 @@ def test_c5_dense_after_compression_hard_overlaps():
 @pytest.mark.parametrize("shape", ["sphere", "halfball"])
 def test_edge_cases(shape):
     import dataclasses
-    base = workloads.config("C1" if shape == "sphere" else "C4", 64 if shape == "halfball" else 48)
+    base = workloads.config("C1" if shape == "sphere" else "C4", 216 if shape == "halfball" else 48)
     pos, quat = workloads.generate(base)
     # (a) no depletants: plain hard-particle MC
     run_parity(base, pos, quat, 10, 0.0)
