@@ -10,6 +10,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -17,6 +18,7 @@
 #include "../../include/hpmc.h"
 #include "cells.cuh"
 #include "move.cuh"
+#include "moveq.cuh"
 
 using namespace hpmc;
 
@@ -60,6 +62,9 @@ struct hpmc_ctx {
   size_t table_rr = 0;
   int num_sms = 148;
   int move_ctas = 0;
+  unsigned int* d_tiles = nullptr;     // 8 tile counters, one per pass of a sweep
+  int q_ctas = 0;                      // persistent CTAs of the item-queue move kernel
+  bool use_queue = true;               // HPMC_MOVE_KERNEL=warp selects the first (warp-per-cell) design
   int64_t launches = 0;
   bool timing = false;
   std::vector<EventPair> ev;
@@ -155,6 +160,35 @@ int get_table(hpmc_ctx* ctx, double lambda, PoissonTable** out) {
   return 0;
 }
 
+constexpr int QT = 256;                // threads (= active cells per tile) of the item-queue kernel
+
+template <int SHAPE>
+int setup_moveq(hpmc_ctx* ctx) {
+  const size_t smem = q_smem_bytes<SHAPE, QT>();
+  cudaError_t e = cudaFuncSetAttribute(k_moveq<SHAPE, QT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  if (e != cudaSuccess) return fail(ctx, HPMC_E_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
+  int per_sm = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_moveq<SHAPE, QT>, QT, smem);
+  if (e != cudaSuccess || per_sm < 1) return fail(ctx, HPMC_E_CUDA, "k_moveq does not fit on an SM");
+  const int ntiles = (ctx->ncell / 8 + QT - 1) / QT;
+  int ctas = ctx->num_sms * per_sm;
+  if (ctas > ntiles) ctas = ntiles;
+  ctx->q_ctas = ctas < 1 ? 1 : ctas;
+  return 0;
+}
+
+template <int SHAPE>
+int launch_moveq(hpmc_ctx* ctx, const MoveArgs& a, int pass) {
+  QArgs q;
+  q.m = a;
+  q.magic_hc = ~0ull / (unsigned long long)a.hc + 1ull;   // floor((2^64-1)/hc)+1 == floor(2^64/hc)+1 unless hc | 2^64
+  if ((a.hc & (a.hc - 1)) == 0) q.magic_hc = (1ull << 63) / (unsigned long long)a.hc * 2ull + 1ull;
+  q.tile_counter = ctx->d_tiles + pass;
+  q.ntiles = (a.nact + QT - 1) / QT;
+  k_moveq<SHAPE, QT><<<ctx->q_ctas, QT, q_smem_bytes<SHAPE, QT>(), ctx->stream>>>(q);
+  return 0;
+}
+
 template <int SHAPE>
 int launch_move(hpmc_ctx* ctx, const MoveArgs& a, bool cb) {
   const dim3 grid(ctx->move_ctas), block(MOVE_WARPS * 32);
@@ -214,6 +248,7 @@ int hpmc_init(hpmc_ctx** out, const hpmc_params* p, int64_t N, float* d_pos4, fl
   CUI(cudaMalloc(&ctx->d_outcome, (size_t)N));
   CUI(cudaMalloc(&ctx->d_counters, sizeof(unsigned long long) * C_COUNT));
   CUI(cudaMalloc(&ctx->d_err, sizeof(int)));
+  CUI(cudaMalloc(&ctx->d_tiles, sizeof(unsigned int) * 8));
   CUI(cudaMemsetAsync(ctx->d_outcome, 0, (size_t)N, ctx->stream));
   CUI(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * C_COUNT, ctx->stream));
   CUI(cudaMemsetAsync(ctx->d_err, 0, sizeof(int), ctx->stream));
@@ -225,6 +260,17 @@ int hpmc_init(hpmc_ctx** out, const hpmc_params* p, int64_t N, float* d_pos4, fl
   if (ctas > need) ctas = need;
   if (ctas < 1) ctas = 1;
   ctx->move_ctas = ctas;
+  {
+    const char* sel = getenv("HPMC_MOVE_KERNEL");
+    ctx->use_queue = !(sel && std::string(sel) == "warp");
+    int rc = 0;
+    switch (p->shape) {
+      case HPMC_SPHERE: rc = setup_moveq<SH_SPHERE>(ctx); break;
+      case HPMC_HALFBALL: rc = setup_moveq<SH_HALFBALL>(ctx); break;
+      default: rc = setup_moveq<SH_SPHERODISK>(ctx); break;
+    }
+    if (rc) { g_init_error = ctx->err; hpmc_destroy(ctx); return rc; }
+  }
   *out = ctx;
   return HPMC_OK;
 }
@@ -235,7 +281,7 @@ void hpmc_destroy(hpmc_ctx* ctx) {
   if (ctx->own_pose) { cudaFree(ctx->d_pos); cudaFree(ctx->d_quat); }
   cudaFree(ctx->d_cpos); cudaFree(ctx->d_caxis); cudaFree(ctx->d_cid); cudaFree(ctx->d_rank);
   cudaFree(ctx->d_cell_pid); cudaFree(ctx->d_counts); cudaFree(ctx->d_cell_start); cudaFree(ctx->d_tile_sums);
-  cudaFree(ctx->d_outcome); cudaFree(ctx->d_counters); cudaFree(ctx->d_err);
+  cudaFree(ctx->d_outcome); cudaFree(ctx->d_counters); cudaFree(ctx->d_err); cudaFree(ctx->d_tiles);
   for (auto& t : ctx->tables) cudaFree(t.d_T);
   for (auto& e : ctx->ev) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   delete ctx;
@@ -294,6 +340,7 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
     const uint32_t t = perm[i]; perm[i] = perm[r]; perm[r] = t;
   }
   CU(cudaMemsetAsync(ctx->d_outcome, 0, (size_t)ctx->N, ctx->stream));
+  CU(cudaMemsetAsync(ctx->d_tiles, 0, sizeof(unsigned int) * 8, ctx->stream));
 
   MoveArgs a;
   a.g = ctx->g; a.key = key;
@@ -317,10 +364,18 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
       ep = &ctx->ev[ctx->ev_used++];
       CU(cudaEventRecord(ep->a, ctx->stream));
     }
-    switch (ctx->p.shape) {
-      case HPMC_SPHERE: launch_move<SH_SPHERE>(ctx, a, cb); break;
-      case HPMC_HALFBALL: launch_move<SH_HALFBALL>(ctx, a, cb); break;
-      default: launch_move<SH_SPHERODISK>(ctx, a, cb); break;
+    if (ctx->use_queue && !cb) {
+      switch (ctx->p.shape) {
+        case HPMC_SPHERE: launch_moveq<SH_SPHERE>(ctx, a, pass); break;
+        case HPMC_HALFBALL: launch_moveq<SH_HALFBALL>(ctx, a, pass); break;
+        default: launch_moveq<SH_SPHERODISK>(ctx, a, pass); break;
+      }
+    } else {
+      switch (ctx->p.shape) {
+        case HPMC_SPHERE: launch_move<SH_SPHERE>(ctx, a, cb); break;
+        case HPMC_HALFBALL: launch_move<SH_HALFBALL>(ctx, a, cb); break;
+        default: launch_move<SH_SPHERODISK>(ctx, a, cb); break;
+      }
     }
     if (ep) CU(cudaEventRecord(ep->b, ctx->stream));
   }

@@ -1,0 +1,377 @@
+// moveq.cuh -- steps a3..a10, second design of the checkerboard move kernel (K-B): "thread per cell + item queue".
+//
+// A CTA of T threads takes tiles of T active cells (dynamic tile counter, persistent CTAs).
+//   phase 1  one THREAD per active cell: pick (a3), trial pose + confinement (a4), walk the 27-cell
+//            neighbourhood once (a5) with the sphere hard-overlap test inline (a6), N_d by table inversion (a7).
+//            Neighbours within r_cut go to a per-move linked list in a CTA-wide shared-memory pool.
+//   phase 1b (convex shapes) the (move, neighbour) pairs inside the circumsphere distance become items; the
+//            CTA's lanes run the support-function test on them side by side.
+//   phase 2  the depletant insertions of ALL surviving moves of the tile are one pool of items
+//            (move m, depletant k, attempt a).  Every lane repeatedly claims the next k of the move it is
+//            attached to (shared-memory atomic), computes ONE Philox block per loop trip, and on an accepted
+//            cube-rejection attempt applies the free-volume test (L68, L72); a rejecting k is folded in with
+//            atomicMin.  A lane whose move is exhausted re-attaches to any unfinished move of the tile, so short
+//            moves (the common case: ~14 needed insertions) cost ~14 lane-items instead of a 32-lane batch, and
+//            long ones (accepted moves test all N_d ~ 2.8k at C3) are shared by up to T lanes.
+//   commit   the owner thread writes outcome, pose, counters (a10).
+// Results are identical to the sequential definition: the outcome depends only on whether a rejecting depletant
+// exists, and dep_needed = (smallest rejecting k) + 1 is exact because k's are claimed in ascending order and a
+// claimed k below the current minimum is never abandoned.
+//
+// PAPER.md: move rule L64-68, Fig. 2 L72; insertion sphere L156; checkerboard + confinement L180; the paper's
+// own GPU layout (App. A: one kernel for trial moves, one thread GROUP per depletant) is prior art.
+#pragma once
+#include <cstdint>
+#include "geometry.cuh"
+#include "move.cuh"
+#include "philox.cuh"
+
+namespace hpmc {
+
+struct QArgs {
+  MoveArgs m;
+  unsigned long long magic_hc;     // floor(2^64 / hc) + 1: exact a / hc by __umul64hi for a < 2^32
+  unsigned int* tile_counter;      // one word per pass, zeroed by the host before the sweep
+  int ntiles;
+};
+
+// s = 2u - 1 with u = ((x >> 9) + 0.5) 2^-23 (R-S4).  Every step is exact in binary32, so this three-instruction
+// form gives the same bits as the (float)(x >> 9) form: f = 1 + n 2^-23, t = f - 1.5, s = 2 t + 2^-23.
+__device__ __forceinline__ float sym_unit_bits(uint32_t x) {
+  const float f = __uint_as_float((x >> 9) | 0x3f800000u);
+  return fmaf(f - 1.5f, 2.0f, 1.1920928955078125e-07f);
+}
+
+template <int SHAPE>
+struct QLayout {
+  static constexpr bool ANISO = SHAPE != SH_SPHERE;
+  static constexpr int ENTRY = ANISO ? 2 : 1;                 // float4 per neighbour entry
+  static constexpr int POOL_PER_SLOT = ANISO ? 12 : 8;        // pool capacity = this x T entries
+  static constexpr int HCAP_PER_SLOT = 4;                     // hard-test items per slot (convex shapes)
+};
+
+template <int SHAPE, int T>
+constexpr size_t q_smem_bytes() {
+  using Lq = QLayout<SHAPE>;
+  size_t b = 0;
+  b += sizeof(float4) * T;                                    // rho_old
+  if (Lq::ANISO) b += sizeof(float4) * T * 2;                 // a_old, a_new
+  b += sizeof(float4) * (size_t)Lq::POOL_PER_SLOT * T * Lq::ENTRY;
+  b += sizeof(uint32_t) * T * 5;                              // pid, Nd, knext, rejmin, head
+  b += sizeof(uint32_t) * (T / 32);                           // todo bitmap
+  b += sizeof(uint16_t) * T;                                  // alive list
+  if (Lq::ANISO) b += sizeof(uint32_t) * Lq::HCAP_PER_SLOT * T + sizeof(uint32_t) * T;   // hard items, hard flags
+  b += 64;                                                    // scalars
+  return b;
+}
+
+template <int SHAPE>
+__device__ __forceinline__ bool q_new_only(const Geo& g, V3 d, V3 rho_old, V3 a_old, V3 a_new) {
+  return dep_overlap<SHAPE>(g, d, a_new) && !dep_overlap<SHAPE>(g, d - rho_old, a_old);
+}
+
+template <int SHAPE>
+__device__ __forceinline__ bool q_free_of_nbrs(const Geo& g, const float4* pool, int head, V3 d) {
+  constexpr int E = QLayout<SHAPE>::ENTRY;
+  for (int e = head; e >= 0;) {
+    const float4 r = pool[e * E];
+    V3 a = V3{0.0f, 0.0f, 1.0f};
+    if (SHAPE != SH_SPHERE) { const float4 t = pool[e * E + 1]; a = V3{t.x, t.y, t.z}; }
+    if (dep_overlap<SHAPE>(g, d - V3{r.x, r.y, r.z}, a)) return false;
+    e = __float_as_int(r.w);
+  }
+  return true;
+}
+
+template <int SHAPE, int T>
+__global__ void __launch_bounds__(T) k_moveq(const QArgs Q) {
+  using Lq = QLayout<SHAPE>;
+  constexpr bool ANISO = Lq::ANISO;
+  constexpr int E = Lq::ENTRY;
+  constexpr int POOL = Lq::POOL_PER_SLOT * T;
+  constexpr int HCAP = Lq::HCAP_PER_SLOT * T;
+  constexpr int NW = T / 32;
+  const MoveArgs& A = Q.m;
+  const Geo& g = A.g;
+
+  extern __shared__ float4 q_smem[];
+  float4* s_rho = q_smem;
+  float4* s_aold = s_rho + T;
+  float4* s_anew = s_aold + (ANISO ? T : 0);
+  float4* s_pool = s_anew + (ANISO ? T : 0);
+  uint32_t* s_pid = reinterpret_cast<uint32_t*>(s_pool + (size_t)POOL * E);
+  uint32_t* s_Nd = s_pid + T;
+  uint32_t* s_knext = s_Nd + T;
+  uint32_t* s_rejmin = s_knext + T;
+  int* s_head = reinterpret_cast<int*>(s_rejmin + T);
+  uint32_t* s_todo = reinterpret_cast<uint32_t*>(s_head + T);
+  uint32_t* s_hitems = s_todo + NW;
+  uint32_t* s_hard = s_hitems + (ANISO ? HCAP : 0);
+  uint32_t* s_scal = s_hard + (ANISO ? T : 0);          // [0] nalive, [1] pool top, [2] tile, [3] n hard items
+  uint16_t* s_alive = reinterpret_cast<uint16_t*>(s_scal + 8);
+
+  const int t = threadIdx.x;
+  const int nc = g.nc, hc = A.hc;
+  const int px = A.colour & 1, py = (A.colour >> 1) & 1, pz = (A.colour >> 2) & 1;
+  const uint32_t colw = A.colour << 8;
+  const uint32_t c3dep = P_DEPPOS + colw;
+
+  // per-thread counters (reduced once at the end of the kernel)
+  uint32_t n_tt = 0, n_at = 0, n_tr = 0, n_ar = 0, n_rb = 0, n_rh = 0, n_rd = 0;
+  uint32_t n_drawn = 0, n_needed = 0, n_eval = 0, n_blocks = 0;
+
+  for (;;) {
+    if (t == 0) {
+      s_scal[2] = atomicAdd(Q.tile_counter, 1u);
+      s_scal[0] = 0; s_scal[1] = 0; s_scal[3] = 0;
+    }
+    __syncthreads();
+    const uint32_t tile = s_scal[2];
+    if (tile >= (uint32_t)Q.ntiles) break;
+
+    // ================================================================ phase 1: one thread per active cell
+    const uint32_t a = tile * T + t;
+    int out = -1;                      // -1: no trial in this slot; OUT_NONE: reached the depletant stage
+    uint32_t pid = 0, slot = 0, Nd = 0;
+    float pw = 0.0f;
+    bool rot = false;
+    V3 r1 = V3{0.f, 0.f, 0.f};
+    Q4 q1 = Q4{1.f, 0.f, 0.f, 0.f};
+    s_head[t] = -1;
+    if (ANISO) s_hard[t] = 0;
+    if (a < (uint32_t)A.nact) {
+      const uint32_t q1d = (uint32_t)__umul64hi((unsigned long long)a, Q.magic_hc);        // a / hc
+      const uint32_t q2d = (uint32_t)__umul64hi((unsigned long long)q1d, Q.magic_hc);      // a / hc^2
+      const int ix = 2 * (int)(a - q1d * hc) + px, iy = 2 * (int)(q1d - q2d * hc) + py, iz = 2 * (int)q2d + pz;
+      const uint32_t cell = ((uint32_t)iz * nc + iy) * nc + ix;
+      const uint32_t cb = A.cell_start[cell], ce = A.cell_start[cell + 1];
+      const uint32_t nocc = ce - cb;
+      if (nocc != 0) {
+        // ---- a3: pick
+        const Block4 rs = philox(A.key, cell, 0, 0, P_SELECT + colw);
+        slot = cb + __umulhi(rs.x, nocc);
+        const float4 p0 = A.cpos[slot];
+        pid = __float_as_uint(p0.w);
+        pw = p0.w;
+        const V3 r0 = V3{p0.x, p0.y, p0.z};
+        Q4 q0 = Q4{1.0f, 0.0f, 0.0f, 0.0f};
+        if (ANISO) q0 = as_q(A.quat[pid]);
+        // ---- a4: trial pose
+        const Block4 rm = philox(A.key, pid, 0, 0, P_MOVE + colw);
+        n_blocks += 2;
+        rot = (A.a_max > 0.0f) && (rm.w & 1u);
+        r1 = r0; q1 = q0;
+        if (!rot) {
+          r1 = V3{wrap1(g, r0.x + A.d_max * sym_unit_bits(rm.x)), wrap1(g, r0.y + A.d_max * sym_unit_bits(rm.y)),
+                  wrap1(g, r0.z + A.d_max * sym_unit_bits(rm.z))};
+          ++n_tt;
+        } else {
+          const V3 v = ball_sample(A.key, pid, 0, 0, P_MOVE + colw + (1u << 16), A.a_max, A.a_max2, n_blocks);
+          q1 = rotate_cayley(q0, v);
+          ++n_tr;
+        }
+        out = OUT_NONE;
+        {
+          const int jx = cell_axis(g, r1.x, A.sx), jy = cell_axis(g, r1.y, A.sy), jz = cell_axis(g, r1.z, A.sz);
+          if (jx != ix || jy != iy || jz != iz) out = OUT_BOUNDARY;
+        }
+        if (out == OUT_NONE) {
+          // ---- a5 + a6: one walk over the 27 cells (9 x-rows; a row is one contiguous span unless it wraps)
+          V3 a_new = V3{0.f, 0.f, 1.f};
+          if (ANISO) a_new = quat_axis(q1);
+          int x0 = ix - 1, n0 = 3, n1 = 0;
+          if (ix == 0) { x0 = nc - 1; n0 = 1; n1 = 2; }
+          else if (ix == nc - 1) { x0 = nc - 2; n0 = 2; n1 = 1; }
+          int head = -1;
+          bool hard = false;
+          for (int row = 0; row < 9 && !hard; ++row) {
+            const int dz = row / 3 - 1, dy = row % 3 - 1;
+            int jy = iy + dy, jz = iz + dz;
+            jy += (jy < 0) ? nc : 0; jy -= (jy >= nc) ? nc : 0;
+            jz += (jz < 0) ? nc : 0; jz -= (jz >= nc) ? nc : 0;
+            const uint32_t rb = ((uint32_t)jz * nc + jy) * nc;
+            for (int seg = 0; seg < 2 && !hard; ++seg) {
+              const int xs = seg ? 0 : x0, nn = seg ? n1 : n0;
+              if (nn == 0) break;
+              const uint32_t sb = A.cell_start[rb + xs], se = A.cell_start[rb + xs + nn];
+              for (uint32_t s = sb; s < se; ++s) {
+                if (s == slot) continue;
+                const float4 pj = A.cpos[s];
+                const V3 rho = V3{minimg1(g, pj.x - r1.x), minimg1(g, pj.y - r1.y), minimg1(g, pj.z - r1.z)};
+                const float r2 = dot3(rho, rho);
+                if (!(r2 < g.rcut2)) continue;
+                if (!ANISO && r2 < g.dcirc2) { hard = true; break; }
+                const int e = (int)atomicAdd(&s_scal[1], 1u);
+                if (e >= POOL) { atomicExch(A.err_flag, 1); continue; }
+                s_pool[e * E] = make_float4(rho.x, rho.y, rho.z, __int_as_float(head));
+                head = e;
+                if (ANISO) {
+                  const float4 axj = A.caxis[s];
+                  s_pool[e * E + 1] = axj;
+                  if (r2 < g.dcirc2) {
+                    const uint32_t hi = atomicAdd(&s_scal[3], 1u);
+                    if (hi < (uint32_t)HCAP) s_hitems[hi] = ((uint32_t)t << 16) | (uint32_t)e;
+                    else if (mpr_overlap<SHAPE>(g, rho, a_new, V3{axj.x, axj.y, axj.z})) hard = true;
+                  }
+                }
+              }
+            }
+          }
+          if (hard) out = OUT_HARD;
+          else {
+            // ---- a7: N_d by table inversion
+            if (A.pt_n > 0) {
+              const Block4 rn = philox(A.key, pid, 0, 0, P_NDEP + colw);
+              ++n_blocks;
+              const unsigned long long U = ((unsigned long long)rn.x << 32) | rn.y;
+              int lo = 0, hi = A.pt_n;
+              while (lo < hi) {
+                const int mid = (lo + hi) >> 1;
+                if (__ldg(&A.ptable[mid]) <= U) lo = mid + 1; else hi = mid;
+              }
+              Nd = A.pt_klo + (uint32_t)lo;
+            }
+            const V3 r0m = V3{minimg1(g, r0.x - r1.x), minimg1(g, r0.y - r1.y), minimg1(g, r0.z - r1.z)};
+            s_rho[t] = make_float4(r0m.x, r0m.y, r0m.z, 0.0f);
+            if (ANISO) {
+              const V3 ao = quat_axis(q0);
+              s_aold[t] = make_float4(ao.x, ao.y, ao.z, 0.0f);
+              s_anew[t] = make_float4(a_new.x, a_new.y, a_new.z, 0.0f);
+            }
+            s_pid[t] = pid; s_Nd[t] = Nd; s_knext[t] = 0; s_rejmin[t] = 0xffffffffu; s_head[t] = head;
+          }
+        }
+      }
+    }
+    // ================================================================ phase 1b: convex hard-overlap items
+    if (ANISO) {
+      __syncthreads();
+      const uint32_t nh = min(s_scal[3], (uint32_t)HCAP);
+      for (uint32_t i = t; i < nh; i += T) {
+        const uint32_t it = s_hitems[i];
+        const uint32_t sl = it >> 16, e = it & 0xffffu;
+        const float4 r = s_pool[e * E], ax = s_pool[e * E + 1], an = s_anew[sl];
+        if (mpr_overlap<SHAPE>(g, V3{r.x, r.y, r.z}, V3{an.x, an.y, an.z}, V3{ax.x, ax.y, ax.z})) s_hard[sl] = 1u;
+      }
+      __syncthreads();
+      if (out == OUT_NONE && s_hard[t]) out = OUT_HARD;
+    }
+    if (out == OUT_NONE) {
+      if (Nd == 0) out = OUT_ACCEPT;
+      else s_alive[atomicAdd(&s_scal[0], 1u)] = (uint16_t)t;
+    }
+    const bool staged = (out == OUT_NONE);
+    __syncthreads();
+    const int nalive = (int)s_scal[0];
+    if (t < NW) {
+      const int rem = nalive - 32 * t;
+      s_todo[t] = rem >= 32 ? 0xffffffffu : (rem > 0 ? ((1u << rem) - 1u) : 0u);
+    }
+    __syncthreads();
+    // ================================================================ phase 2: depletant items (a8)
+    if (nalive > 0) {
+      int j = t % nalive;
+      uint32_t m = s_alive[j];
+      uint32_t c_pid = s_pid[m], c_Nd = s_Nd[m];
+      int c_head = s_head[m];
+      float4 c_rho = s_rho[m];
+      V3 c_aold = V3{0.f, 0.f, 1.f}, c_anew = V3{0.f, 0.f, 1.f};
+      if (ANISO) {
+        const float4 ao = s_aold[m], an = s_anew[m];
+        c_aold = V3{ao.x, ao.y, ao.z}; c_anew = V3{an.x, an.y, an.z};
+      }
+      volatile uint32_t* v_rejmin = s_rejmin;
+      volatile uint32_t* v_todo = s_todo;
+      uint32_t k = 0, att = 0;
+      bool have = false, active = true;
+      while (active) {
+        while (!have) {
+          k = atomicAdd(&s_knext[m], 1u);
+          const uint32_t lim = min(c_Nd, v_rejmin[m]);
+          if (k < lim) { att = 0; have = true; break; }
+          // this move has no unclaimed work left: retire its bit and attach to an unfinished move of the tile
+          atomicAnd(&s_todo[j >> 5], ~(1u << (j & 31)));
+          int found = -1;
+#pragma unroll 1
+          for (int i = 0; i < NW; ++i) {
+            const int wi = ((j >> 5) + i) % NW;
+            const uint32_t w = v_todo[wi];
+            if (w) {
+              const int r = t & 31;
+              const uint32_t w2 = __funnelshift_r(w, w, r);
+              found = wi * 32 + ((__ffs(w2) - 1 + r) & 31);
+              break;
+            }
+          }
+          if (found < 0) { active = false; break; }
+          j = found;
+          m = s_alive[j];
+          c_pid = s_pid[m]; c_Nd = s_Nd[m]; c_head = s_head[m]; c_rho = s_rho[m];
+          if (ANISO) {
+            const float4 ao = s_aold[m], an = s_anew[m];
+            c_aold = V3{ao.x, ao.y, ao.z}; c_anew = V3{an.x, an.y, an.z};
+          }
+        }
+        if (!active) break;
+        // one Philox block = one cube-rejection attempt of depletant k (R-S3)
+        const Block4 r = philox(A.key, c_pid, k, 0, c3dep + (att << 16));
+        ++n_blocks;
+        V3 d = V3{g.Rins * sym_unit_bits(r.x), g.Rins * sym_unit_bits(r.y), g.Rins * sym_unit_bits(r.z)};
+        bool inside = dot3(d, d) <= g.Rins2;
+        if (!inside && att == 63u) { d = V3{0.f, 0.f, 0.f}; inside = true; }
+        if (inside) {
+          ++n_eval;
+          const V3 ro = V3{c_rho.x, c_rho.y, c_rho.z};
+          if (q_new_only<SHAPE>(g, d, ro, c_aold, c_anew) && q_free_of_nbrs<SHAPE>(g, s_pool, c_head, d))
+            atomicMin(&s_rejmin[m], k);
+          have = false;
+        } else {
+          ++att;
+          if (k > v_rejmin[m]) have = false;       // a lower k already rejects: this one cannot matter
+        }
+      }
+    }
+    __syncthreads();
+    // ================================================================ commit (a10)
+    if (out != -1) {
+      if (staged) {
+        const uint32_t rm_ = s_rejmin[t];
+        const bool rej = rm_ < Nd;
+        out = rej ? OUT_DEPLETANT : OUT_ACCEPT;
+        n_drawn += Nd;
+        n_needed += rej ? rm_ + 1u : Nd;
+      }
+      A.outcome[pid] = (uint8_t)out;
+      if (out == OUT_ACCEPT) {
+        float4 pn = A.pos[pid];
+        pn.x = r1.x; pn.y = r1.y; pn.z = r1.z;
+        A.pos[pid] = pn;
+        A.cpos[slot] = make_float4(r1.x, r1.y, r1.z, pw);
+        if (ANISO && rot) {
+          A.quat[pid] = as_f4(q1);
+          const V3 an = quat_axis(q1);
+          A.caxis[slot] = make_float4(an.x, an.y, an.z, 0.0f);
+        }
+        if (rot) ++n_ar; else ++n_at;
+      } else if (out == OUT_BOUNDARY) ++n_rb;
+      else if (out == OUT_HARD) ++n_rh;
+      else ++n_rd;
+    }
+    __syncthreads();
+  }
+
+  // ---- counters: warp reduction, one atomic per warp and counter
+  const unsigned FULL = 0xffffffffu;
+  unsigned long long v[11] = {n_tt, n_at, n_tr, n_ar, n_rb, n_rh, n_rd, n_drawn, n_needed, n_eval, n_blocks};
+  const int idx[11] = {C_TRIALS_TRANS, C_ACCEPT_TRANS, C_TRIALS_ROT, C_ACCEPT_ROT, C_REJ_BOUNDARY, C_REJ_HARD,
+                       C_REJ_DEPLETANT, C_DEP_DRAWN, C_DEP_NEEDED, C_DEP_EVALUATED, C_PHILOX_BLOCKS};
+#pragma unroll
+  for (int c = 0; c < 11; ++c) {
+    unsigned long long x = v[c];
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) x += __shfl_xor_sync(FULL, x, o);
+    if ((t & 31) == 0 && x) atomicAdd(&A.counters[idx[c]], x);
+  }
+}
+
+}  // namespace hpmc
