@@ -160,17 +160,18 @@ int get_table(hpmc_ctx* ctx, double lambda, PoissonTable** out) {
   return 0;
 }
 
-constexpr int QT = 256;                // threads (= active cells per tile) of the item-queue kernel
+constexpr int QT = 128;                // threads per CTA of the item-queue kernel
+constexpr int QCPT = 2;                // active cells per thread and tile
 
 template <int SHAPE>
 int setup_moveq(hpmc_ctx* ctx) {
-  const size_t smem = q_smem_bytes<SHAPE, QT>();
-  cudaError_t e = cudaFuncSetAttribute(k_moveq<SHAPE, QT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  const size_t smem = QSmem<SHAPE, QT, QCPT>::bytes;
+  cudaError_t e = cudaFuncSetAttribute(k_moveq<SHAPE, QT, QCPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return fail(ctx, HPMC_E_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
   int per_sm = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_moveq<SHAPE, QT>, QT, smem);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_moveq<SHAPE, QT, QCPT>, QT, smem);
   if (e != cudaSuccess || per_sm < 1) return fail(ctx, HPMC_E_CUDA, "k_moveq does not fit on an SM");
-  const int ntiles = (ctx->ncell / 8 + QT - 1) / QT;
+  const int ntiles = (ctx->ncell / 8 + QT * QCPT - 1) / (QT * QCPT);
   int ctas = ctx->num_sms * per_sm;
   if (ctas > ntiles) ctas = ntiles;
   ctx->q_ctas = ctas < 1 ? 1 : ctas;
@@ -184,8 +185,13 @@ int launch_moveq(hpmc_ctx* ctx, const MoveArgs& a, int pass) {
   q.magic_hc = ~0ull / (unsigned long long)a.hc + 1ull;   // floor((2^64-1)/hc)+1 == floor(2^64/hc)+1 unless hc | 2^64
   if ((a.hc & (a.hc - 1)) == 0) q.magic_hc = (1ull << 63) / (unsigned long long)a.hc * 2ull + 1ull;
   q.tile_counter = ctx->d_tiles + pass;
-  q.ntiles = (a.nact + QT - 1) / QT;
-  k_moveq<SHAPE, QT><<<ctx->q_ctas, QT, q_smem_bytes<SHAPE, QT>(), ctx->stream>>>(q);
+  q.ntiles = (a.nact + QT * QCPT - 1) / (QT * QCPT);
+  {
+    const float rl = (ctx->p.sigma_c + ctx->p.sigma_d) + 1e-3f;
+    q.rlist2 = rl * rl;
+    if (q.rlist2 > a.g.rcut2) q.rlist2 = a.g.rcut2;
+  }
+  k_moveq<SHAPE, QT, QCPT><<<ctx->q_ctas, QT, QSmem<SHAPE, QT, QCPT>::bytes, ctx->stream>>>(q);
   return 0;
 }
 

@@ -1,10 +1,13 @@
 // moveq.cuh -- steps a3..a10, second design of the checkerboard move kernel (K-B): "thread per cell + item queue".
 //
-// A CTA of T threads takes tiles of T active cells (dynamic tile counter, persistent CTAs).
-//   phase 1  one THREAD per active cell: pick (a3), trial pose + confinement (a4), walk the 27-cell
-//            neighbourhood once (a5) with the sphere hard-overlap test inline (a6), N_d by table inversion (a7).
-//            Neighbours within r_cut go to a per-move linked list in a CTA-wide shared-memory pool.
-//   phase 1b (convex shapes) the (move, neighbour) pairs inside the circumsphere distance become items; the
+// A CTA of T threads takes tiles of CPT*T active cells (dynamic tile counter, persistent CTAs).
+//   phase 1a one THREAD per active cell (CPT cells each): pick (a3), trial pose + confinement (a4).  Moves that
+//            stay in their cell are compacted into a dense list in shared memory (empty cells and boundary
+//            rejections -- about half of the cells at C3 -- drop out here).
+//   phase 1b one thread per listed move: one walk over the 27-cell neighbourhood (a5) with the sphere
+//            hard-overlap test inline (a6), then N_d by table inversion (a7).  Neighbours that a depletant of
+//            this move can touch go to a per-move linked list in a CTA-wide shared-memory pool.
+//   phase 1c (convex shapes) the (move, neighbour) pairs inside the circumsphere distance become items; the
 //            CTA's lanes run the support-function test on them side by side.
 //   phase 2  the depletant insertions of ALL surviving moves of the tile are one pool of items
 //            (move m, depletant k, attempt a).  Every lane repeatedly claims the next k of the move it is
@@ -33,6 +36,9 @@ struct QArgs {
   unsigned long long magic_hc;     // floor(2^64 / hc) + 1: exact a / hc by __umul64hi for a < 2^32
   unsigned int* tile_counter;      // one word per pass, zeroed by the host before the sweep
   int ntiles;
+  float rlist2;                    // neighbours farther than this from the new centre cannot touch any depletant
+                                   // of the move: (sigma_c + sigma_d + 1e-3)^2 for the plain rule (insertion
+                                   // sphere about the new centre only), r_cut^2 of R-3.4 otherwise
 };
 
 // s = 2u - 1 with u = ((x >> 9) + 0.5) 2^-23 (R-S4).  Every step is exact in binary32, so this three-instruction
@@ -46,24 +52,35 @@ template <int SHAPE>
 struct QLayout {
   static constexpr bool ANISO = SHAPE != SH_SPHERE;
   static constexpr int ENTRY = ANISO ? 2 : 1;                 // float4 per neighbour entry
-  static constexpr int POOL_PER_SLOT = ANISO ? 12 : 8;        // pool capacity = this x T entries
-  static constexpr int HCAP_PER_SLOT = 4;                     // hard-test items per slot (convex shapes)
+  static constexpr int POOL_PER_THREAD = ANISO ? 12 : 8;      // pool capacity = this x T entries
+  static constexpr int HCAP_PER_THREAD = 4;                   // hard-test items (convex shapes) = this x T
 };
 
-template <int SHAPE, int T>
-constexpr size_t q_smem_bytes() {
+// shared-memory carve-up for a CTA of T threads handling M = CPT*T cells per tile
+template <int SHAPE, int T, int CPT>
+struct QSmem {
   using Lq = QLayout<SHAPE>;
-  size_t b = 0;
-  b += sizeof(float4) * T;                                    // rho_old
-  if (Lq::ANISO) b += sizeof(float4) * T * 2;                 // a_old, a_new
-  b += sizeof(float4) * (size_t)Lq::POOL_PER_SLOT * T * Lq::ENTRY;
-  b += sizeof(uint32_t) * T * 5;                              // pid, Nd, knext, rejmin, head
-  b += sizeof(uint32_t) * (T / 32);                           // todo bitmap
-  b += sizeof(uint16_t) * T;                                  // alive list
-  if (Lq::ANISO) b += sizeof(uint32_t) * Lq::HCAP_PER_SLOT * T + sizeof(uint32_t) * T;   // hard items, hard flags
-  b += 64;                                                    // scalars
-  return b;
-}
+  static constexpr int M = CPT * T;
+  static constexpr int POOL = Lq::POOL_PER_THREAD * T;
+  static constexpr int HCAP = Lq::ANISO ? Lq::HCAP_PER_THREAD * T : 0;
+  static constexpr size_t o_r1 = 0;                                             // float4[M]  r1.xyz, pid bits
+  static constexpr size_t o_rho = o_r1 + sizeof(float4) * M;                    // float4[M]  rho_old.xyz, slot bits
+  static constexpr size_t o_q1 = o_rho + sizeof(float4) * M;                    // float4[M]  new quaternion (aniso)
+  static constexpr size_t o_aold = o_q1 + (Lq::ANISO ? sizeof(float4) * M : 0); // float4[M]
+  static constexpr size_t o_anew = o_aold + (Lq::ANISO ? sizeof(float4) * M : 0);
+  static constexpr size_t o_pool = o_anew + (Lq::ANISO ? sizeof(float4) * M : 0);
+  static constexpr size_t o_cell = o_pool + sizeof(float4) * (size_t)POOL * Lq::ENTRY;   // u32[M] ix|iy<<10|iz<<20|rot<<30
+  static constexpr size_t o_Nd = o_cell + 4 * M;
+  static constexpr size_t o_knext = o_Nd + 4 * M;
+  static constexpr size_t o_rejmin = o_knext + 4 * M;
+  static constexpr size_t o_head = o_rejmin + 4 * M;
+  static constexpr size_t o_state = o_head + 4 * M;                             // u32[M] outcome code so far
+  static constexpr size_t o_todo = o_state + 4 * M;                             // u32[M/32]
+  static constexpr size_t o_hitems = o_todo + 4 * (M / 32);
+  static constexpr size_t o_scal = o_hitems + 4 * HCAP;                         // u32[8]
+  static constexpr size_t o_alive = o_scal + 32;                                // u16[M]
+  static constexpr size_t bytes = o_alive + 2 * M;
+};
 
 template <int SHAPE>
 __device__ __forceinline__ bool q_new_only(const Geo& g, V3 d, V3 rho_old, V3 a_old, V3 a_new) {
@@ -83,32 +100,34 @@ __device__ __forceinline__ bool q_free_of_nbrs(const Geo& g, const float4* pool,
   return true;
 }
 
-template <int SHAPE, int T>
+template <int SHAPE, int T, int CPT>
 __global__ void __launch_bounds__(T) k_moveq(const QArgs Q) {
   using Lq = QLayout<SHAPE>;
+  using S = QSmem<SHAPE, T, CPT>;
   constexpr bool ANISO = Lq::ANISO;
   constexpr int E = Lq::ENTRY;
-  constexpr int POOL = Lq::POOL_PER_SLOT * T;
-  constexpr int HCAP = Lq::HCAP_PER_SLOT * T;
-  constexpr int NW = T / 32;
+  constexpr int M = S::M, POOL = S::POOL, HCAP = S::HCAP, NW = M / 32;
   const MoveArgs& A = Q.m;
   const Geo& g = A.g;
 
   extern __shared__ float4 q_smem[];
-  float4* s_rho = q_smem;
-  float4* s_aold = s_rho + T;
-  float4* s_anew = s_aold + (ANISO ? T : 0);
-  float4* s_pool = s_anew + (ANISO ? T : 0);
-  uint32_t* s_pid = reinterpret_cast<uint32_t*>(s_pool + (size_t)POOL * E);
-  uint32_t* s_Nd = s_pid + T;
-  uint32_t* s_knext = s_Nd + T;
-  uint32_t* s_rejmin = s_knext + T;
-  int* s_head = reinterpret_cast<int*>(s_rejmin + T);
-  uint32_t* s_todo = reinterpret_cast<uint32_t*>(s_head + T);
-  uint32_t* s_hitems = s_todo + NW;
-  uint32_t* s_hard = s_hitems + (ANISO ? HCAP : 0);
-  uint32_t* s_scal = s_hard + (ANISO ? T : 0);          // [0] nalive, [1] pool top, [2] tile, [3] n hard items
-  uint16_t* s_alive = reinterpret_cast<uint16_t*>(s_scal + 8);
+  char* sb_ = reinterpret_cast<char*>(q_smem);
+  float4* s_r1 = reinterpret_cast<float4*>(sb_ + S::o_r1);
+  float4* s_rho = reinterpret_cast<float4*>(sb_ + S::o_rho);
+  float4* s_q1 = reinterpret_cast<float4*>(sb_ + S::o_q1);
+  float4* s_aold = reinterpret_cast<float4*>(sb_ + S::o_aold);
+  float4* s_anew = reinterpret_cast<float4*>(sb_ + S::o_anew);
+  float4* s_pool = reinterpret_cast<float4*>(sb_ + S::o_pool);
+  uint32_t* s_cell = reinterpret_cast<uint32_t*>(sb_ + S::o_cell);
+  uint32_t* s_Nd = reinterpret_cast<uint32_t*>(sb_ + S::o_Nd);
+  uint32_t* s_knext = reinterpret_cast<uint32_t*>(sb_ + S::o_knext);
+  uint32_t* s_rejmin = reinterpret_cast<uint32_t*>(sb_ + S::o_rejmin);
+  int* s_head = reinterpret_cast<int*>(sb_ + S::o_head);
+  uint32_t* s_state = reinterpret_cast<uint32_t*>(sb_ + S::o_state);
+  uint32_t* s_todo = reinterpret_cast<uint32_t*>(sb_ + S::o_todo);
+  uint32_t* s_hitems = reinterpret_cast<uint32_t*>(sb_ + S::o_hitems);
+  uint32_t* s_scal = reinterpret_cast<uint32_t*>(sb_ + S::o_scal);   // [0] nalive [1] pool top [2] tile [3] nhard [4] nlist
+  uint16_t* s_alive = reinterpret_cast<uint16_t*>(sb_ + S::o_alive);
 
   const int t = threadIdx.x;
   const int nc = g.nc, hc = A.hc;
@@ -123,156 +142,162 @@ __global__ void __launch_bounds__(T) k_moveq(const QArgs Q) {
   for (;;) {
     if (t == 0) {
       s_scal[2] = atomicAdd(Q.tile_counter, 1u);
-      s_scal[0] = 0; s_scal[1] = 0; s_scal[3] = 0;
+      s_scal[0] = 0; s_scal[1] = 0; s_scal[3] = 0; s_scal[4] = 0;
     }
     __syncthreads();
     const uint32_t tile = s_scal[2];
     if (tile >= (uint32_t)Q.ntiles) break;
 
-    // ================================================================ phase 1: one thread per active cell
-    const uint32_t a = tile * T + t;
-    int out = -1;                      // -1: no trial in this slot; OUT_NONE: reached the depletant stage
-    uint32_t pid = 0, slot = 0, Nd = 0;
-    float pw = 0.0f;
-    bool rot = false;
-    V3 r1 = V3{0.f, 0.f, 0.f};
-    Q4 q1 = Q4{1.f, 0.f, 0.f, 0.f};
-    s_head[t] = -1;
-    if (ANISO) s_hard[t] = 0;
-    if (a < (uint32_t)A.nact) {
+    // ================================================================ phase 1a: one thread per active cell
+#pragma unroll 1
+    for (int c = 0; c < CPT; ++c) {
+      const uint32_t a = tile * M + c * T + t;
+      if (a >= (uint32_t)A.nact) continue;
       const uint32_t q1d = (uint32_t)__umul64hi((unsigned long long)a, Q.magic_hc);        // a / hc
       const uint32_t q2d = (uint32_t)__umul64hi((unsigned long long)q1d, Q.magic_hc);      // a / hc^2
       const int ix = 2 * (int)(a - q1d * hc) + px, iy = 2 * (int)(q1d - q2d * hc) + py, iz = 2 * (int)q2d + pz;
       const uint32_t cell = ((uint32_t)iz * nc + iy) * nc + ix;
       const uint32_t cb = A.cell_start[cell], ce = A.cell_start[cell + 1];
       const uint32_t nocc = ce - cb;
-      if (nocc != 0) {
-        // ---- a3: pick
-        const Block4 rs = philox(A.key, cell, 0, 0, P_SELECT + colw);
-        slot = cb + __umulhi(rs.x, nocc);
-        const float4 p0 = A.cpos[slot];
-        pid = __float_as_uint(p0.w);
-        pw = p0.w;
-        const V3 r0 = V3{p0.x, p0.y, p0.z};
-        Q4 q0 = Q4{1.0f, 0.0f, 0.0f, 0.0f};
-        if (ANISO) q0 = as_q(A.quat[pid]);
-        // ---- a4: trial pose
-        const Block4 rm = philox(A.key, pid, 0, 0, P_MOVE + colw);
-        n_blocks += 2;
-        rot = (A.a_max > 0.0f) && (rm.w & 1u);
-        r1 = r0; q1 = q0;
-        if (!rot) {
-          r1 = V3{wrap1(g, r0.x + A.d_max * sym_unit_bits(rm.x)), wrap1(g, r0.y + A.d_max * sym_unit_bits(rm.y)),
-                  wrap1(g, r0.z + A.d_max * sym_unit_bits(rm.z))};
-          ++n_tt;
-        } else {
-          const V3 v = ball_sample(A.key, pid, 0, 0, P_MOVE + colw + (1u << 16), A.a_max, A.a_max2, n_blocks);
-          q1 = rotate_cayley(q0, v);
-          ++n_tr;
-        }
-        out = OUT_NONE;
-        {
-          const int jx = cell_axis(g, r1.x, A.sx), jy = cell_axis(g, r1.y, A.sy), jz = cell_axis(g, r1.z, A.sz);
-          if (jx != ix || jy != iy || jz != iz) out = OUT_BOUNDARY;
-        }
-        if (out == OUT_NONE) {
-          // ---- a5 + a6: one walk over the 27 cells (9 x-rows; a row is one contiguous span unless it wraps)
-          V3 a_new = V3{0.f, 0.f, 1.f};
-          if (ANISO) a_new = quat_axis(q1);
-          int x0 = ix - 1, n0 = 3, n1 = 0;
-          if (ix == 0) { x0 = nc - 1; n0 = 1; n1 = 2; }
-          else if (ix == nc - 1) { x0 = nc - 2; n0 = 2; n1 = 1; }
-          int head = -1;
-          bool hard = false;
-          for (int row = 0; row < 9 && !hard; ++row) {
-            const int dz = row / 3 - 1, dy = row % 3 - 1;
-            int jy = iy + dy, jz = iz + dz;
-            jy += (jy < 0) ? nc : 0; jy -= (jy >= nc) ? nc : 0;
-            jz += (jz < 0) ? nc : 0; jz -= (jz >= nc) ? nc : 0;
-            const uint32_t rb = ((uint32_t)jz * nc + jy) * nc;
-            for (int seg = 0; seg < 2 && !hard; ++seg) {
-              const int xs = seg ? 0 : x0, nn = seg ? n1 : n0;
-              if (nn == 0) break;
-              const uint32_t sb = A.cell_start[rb + xs], se = A.cell_start[rb + xs + nn];
-              for (uint32_t s = sb; s < se; ++s) {
-                if (s == slot) continue;
-                const float4 pj = A.cpos[s];
-                const V3 rho = V3{minimg1(g, pj.x - r1.x), minimg1(g, pj.y - r1.y), minimg1(g, pj.z - r1.z)};
-                const float r2 = dot3(rho, rho);
-                if (!(r2 < g.rcut2)) continue;
-                if (!ANISO && r2 < g.dcirc2) { hard = true; break; }
-                const int e = (int)atomicAdd(&s_scal[1], 1u);
-                if (e >= POOL) { atomicExch(A.err_flag, 1); continue; }
-                s_pool[e * E] = make_float4(rho.x, rho.y, rho.z, __int_as_float(head));
-                head = e;
-                if (ANISO) {
-                  const float4 axj = A.caxis[s];
-                  s_pool[e * E + 1] = axj;
-                  if (r2 < g.dcirc2) {
-                    const uint32_t hi = atomicAdd(&s_scal[3], 1u);
-                    if (hi < (uint32_t)HCAP) s_hitems[hi] = ((uint32_t)t << 16) | (uint32_t)e;
-                    else if (mpr_overlap<SHAPE>(g, rho, a_new, V3{axj.x, axj.y, axj.z})) hard = true;
-                  }
-                }
-              }
-            }
-          }
-          if (hard) out = OUT_HARD;
-          else {
-            // ---- a7: N_d by table inversion
-            if (A.pt_n > 0) {
-              const Block4 rn = philox(A.key, pid, 0, 0, P_NDEP + colw);
-              ++n_blocks;
-              const unsigned long long U = ((unsigned long long)rn.x << 32) | rn.y;
-              int lo = 0, hi = A.pt_n;
-              while (lo < hi) {
-                const int mid = (lo + hi) >> 1;
-                if (__ldg(&A.ptable[mid]) <= U) lo = mid + 1; else hi = mid;
-              }
-              Nd = A.pt_klo + (uint32_t)lo;
-            }
-            const V3 r0m = V3{minimg1(g, r0.x - r1.x), minimg1(g, r0.y - r1.y), minimg1(g, r0.z - r1.z)};
-            s_rho[t] = make_float4(r0m.x, r0m.y, r0m.z, 0.0f);
+      if (nocc == 0) continue;
+      // ---- a3: pick
+      const Block4 rs = philox(A.key, cell, 0, 0, P_SELECT + colw);
+      const uint32_t slot = cb + __umulhi(rs.x, nocc);
+      const float4 p0 = A.cpos[slot];
+      const uint32_t pid = __float_as_uint(p0.w);
+      const V3 r0 = V3{p0.x, p0.y, p0.z};
+      Q4 q0 = Q4{1.0f, 0.0f, 0.0f, 0.0f};
+      if (ANISO) q0 = as_q(A.quat[pid]);
+      // ---- a4: trial pose
+      const Block4 rm = philox(A.key, pid, 0, 0, P_MOVE + colw);
+      n_blocks += 2;
+      const bool rot = (A.a_max > 0.0f) && (rm.w & 1u);
+      V3 r1 = r0;
+      Q4 q1 = q0;
+      if (!rot) {
+        r1 = V3{wrap1(g, r0.x + A.d_max * sym_unit_bits(rm.x)), wrap1(g, r0.y + A.d_max * sym_unit_bits(rm.y)),
+                wrap1(g, r0.z + A.d_max * sym_unit_bits(rm.z))};
+        ++n_tt;
+      } else {
+        const V3 v = ball_sample(A.key, pid, 0, 0, P_MOVE + colw + (1u << 16), A.a_max, A.a_max2, n_blocks);
+        q1 = rotate_cayley(q0, v);
+        ++n_tr;
+      }
+      const int jx = cell_axis(g, r1.x, A.sx), jy = cell_axis(g, r1.y, A.sy), jz = cell_axis(g, r1.z, A.sz);
+      if (jx != ix || jy != iy || jz != iz) {        // confinement (L180)
+        A.outcome[pid] = (uint8_t)OUT_BOUNDARY;
+        ++n_rb;
+        continue;
+      }
+      const uint32_t e = atomicAdd(&s_scal[4], 1u);
+      s_r1[e] = make_float4(r1.x, r1.y, r1.z, p0.w);
+      s_rho[e] = make_float4(minimg1(g, r0.x - r1.x), minimg1(g, r0.y - r1.y), minimg1(g, r0.z - r1.z),
+                             __uint_as_float(slot));
+      s_cell[e] = (uint32_t)ix | ((uint32_t)iy << 10) | ((uint32_t)iz << 20) | (rot ? (1u << 30) : 0u);
+      if (ANISO) {
+        s_q1[e] = as_f4(q1);
+        const V3 ao = quat_axis(q0), an = quat_axis(q1);
+        s_aold[e] = make_float4(ao.x, ao.y, ao.z, 0.0f);
+        s_anew[e] = make_float4(an.x, an.y, an.z, 0.0f);
+      }
+    }
+    __syncthreads();
+    const int nlist = (int)s_scal[4];
+
+    // ================================================================ phase 1b: one thread per listed move
+#pragma unroll 1
+    for (int e = t; e < nlist; e += T) {
+      const float4 r1f = s_r1[e];
+      const V3 r1 = V3{r1f.x, r1f.y, r1f.z};
+      const uint32_t pid = __float_as_uint(r1f.w);
+      const uint32_t slot = __float_as_uint(s_rho[e].w);
+      const uint32_t cw = s_cell[e];
+      const int ix = cw & 1023, iy = (cw >> 10) & 1023, iz = (cw >> 20) & 1023;
+      V3 a_new = V3{0.f, 0.f, 1.f};
+      if (ANISO) { const float4 an = s_anew[e]; a_new = V3{an.x, an.y, an.z}; }
+      // ---- a5 + a6: one walk over the 27 cells (9 x-rows; a row is one contiguous span unless it wraps)
+      int x0 = ix - 1, n0 = 3, n1 = 0;
+      if (ix == 0) { x0 = nc - 1; n0 = 1; n1 = 2; }
+      else if (ix == nc - 1) { x0 = nc - 2; n0 = 2; n1 = 1; }
+      int head = -1;
+      bool hard = false;
+      for (int row = 0; row < 9 && !hard; ++row) {
+        const int dz = row / 3 - 1, dy = row % 3 - 1;
+        int jy = iy + dy, jz = iz + dz;
+        jy += (jy < 0) ? nc : 0; jy -= (jy >= nc) ? nc : 0;
+        jz += (jz < 0) ? nc : 0; jz -= (jz >= nc) ? nc : 0;
+        const uint32_t rb = ((uint32_t)jz * nc + jy) * nc;
+        for (int seg = 0; seg < 2 && !hard; ++seg) {
+          const int xs = seg ? 0 : x0, nn = seg ? n1 : n0;
+          if (nn == 0) break;
+          const uint32_t sb = A.cell_start[rb + xs], se = A.cell_start[rb + xs + nn];
+          for (uint32_t s = sb; s < se; ++s) {
+            if (s == slot) continue;
+            const float4 pj = A.cpos[s];
+            const V3 rho = V3{minimg1(g, pj.x - r1.x), minimg1(g, pj.y - r1.y), minimg1(g, pj.z - r1.z)};
+            const float r2 = dot3(rho, rho);
+            if (!(r2 < Q.rlist2)) continue;
+            if (!ANISO && r2 < g.dcirc2) { hard = true; break; }
+            const int pe = (int)atomicAdd(&s_scal[1], 1u);
+            if (pe >= POOL) { atomicExch(A.err_flag, 1); continue; }
+            s_pool[pe * E] = make_float4(rho.x, rho.y, rho.z, __int_as_float(head));
+            head = pe;
             if (ANISO) {
-              const V3 ao = quat_axis(q0);
-              s_aold[t] = make_float4(ao.x, ao.y, ao.z, 0.0f);
-              s_anew[t] = make_float4(a_new.x, a_new.y, a_new.z, 0.0f);
+              const float4 axj = A.caxis[s];
+              s_pool[pe * E + 1] = axj;
+              if (r2 < g.dcirc2) {
+                const uint32_t hi = atomicAdd(&s_scal[3], 1u);
+                if (hi < (uint32_t)HCAP) s_hitems[hi] = ((uint32_t)e << 16) | (uint32_t)pe;
+                else if (mpr_overlap<SHAPE>(g, rho, a_new, V3{axj.x, axj.y, axj.z})) hard = true;
+              }
             }
-            s_pid[t] = pid; s_Nd[t] = Nd; s_knext[t] = 0; s_rejmin[t] = 0xffffffffu; s_head[t] = head;
           }
         }
       }
+      uint32_t Nd = 0;
+      if (!hard && A.pt_n > 0) {
+        // ---- a7: N_d by table inversion
+        const Block4 rn = philox(A.key, pid, 0, 0, P_NDEP + colw);
+        ++n_blocks;
+        const unsigned long long U = ((unsigned long long)rn.x << 32) | rn.y;
+        int lo = 0, hi = A.pt_n;
+        while (lo < hi) {
+          const int mid = (lo + hi) >> 1;
+          if (__ldg(&A.ptable[mid]) <= U) lo = mid + 1; else hi = mid;
+        }
+        Nd = A.pt_klo + (uint32_t)lo;
+      }
+      s_Nd[e] = Nd; s_knext[e] = 0; s_rejmin[e] = 0xffffffffu; s_head[e] = head;
+      s_state[e] = hard ? OUT_HARD : OUT_NONE;
+      if (!ANISO && !hard && Nd != 0) s_alive[atomicAdd(&s_scal[0], 1u)] = (uint16_t)e;
     }
-    // ================================================================ phase 1b: convex hard-overlap items
+    // ================================================================ phase 1c: convex hard-overlap items
     if (ANISO) {
       __syncthreads();
       const uint32_t nh = min(s_scal[3], (uint32_t)HCAP);
       for (uint32_t i = t; i < nh; i += T) {
         const uint32_t it = s_hitems[i];
-        const uint32_t sl = it >> 16, e = it & 0xffffu;
-        const float4 r = s_pool[e * E], ax = s_pool[e * E + 1], an = s_anew[sl];
-        if (mpr_overlap<SHAPE>(g, V3{r.x, r.y, r.z}, V3{an.x, an.y, an.z}, V3{ax.x, ax.y, ax.z})) s_hard[sl] = 1u;
+        const uint32_t sl = it >> 16, pe = it & 0xffffu;
+        const float4 r = s_pool[pe * E], ax = s_pool[pe * E + 1], an = s_anew[sl];
+        if (mpr_overlap<SHAPE>(g, V3{r.x, r.y, r.z}, V3{an.x, an.y, an.z}, V3{ax.x, ax.y, ax.z}))
+          s_state[sl] = OUT_HARD;
       }
       __syncthreads();
-      if (out == OUT_NONE && s_hard[t]) out = OUT_HARD;
+      for (int e = t; e < nlist; e += T)
+        if (s_state[e] == OUT_NONE && s_Nd[e] != 0) s_alive[atomicAdd(&s_scal[0], 1u)] = (uint16_t)e;
     }
-    if (out == OUT_NONE) {
-      if (Nd == 0) out = OUT_ACCEPT;
-      else s_alive[atomicAdd(&s_scal[0], 1u)] = (uint16_t)t;
-    }
-    const bool staged = (out == OUT_NONE);
     __syncthreads();
     const int nalive = (int)s_scal[0];
-    if (t < NW) {
-      const int rem = nalive - 32 * t;
-      s_todo[t] = rem >= 32 ? 0xffffffffu : (rem > 0 ? ((1u << rem) - 1u) : 0u);
+    for (int w = t; w < NW; w += T) {
+      const int rem = nalive - 32 * w;
+      s_todo[w] = rem >= 32 ? 0xffffffffu : (rem > 0 ? ((1u << rem) - 1u) : 0u);
     }
     __syncthreads();
     // ================================================================ phase 2: depletant items (a8)
     if (nalive > 0) {
       int j = t % nalive;
       uint32_t m = s_alive[j];
-      uint32_t c_pid = s_pid[m], c_Nd = s_Nd[m];
+      uint32_t c_pid = __float_as_uint(s_r1[m].w), c_Nd = s_Nd[m];
       int c_head = s_head[m];
       float4 c_rho = s_rho[m];
       V3 c_aold = V3{0.f, 0.f, 1.f}, c_anew = V3{0.f, 0.f, 1.f};
@@ -284,58 +309,69 @@ __global__ void __launch_bounds__(T) k_moveq(const QArgs Q) {
       volatile uint32_t* v_todo = s_todo;
       uint32_t k = 0, att = 0;
       bool have = false, active = true;
-      while (active) {
-        while (!have) {
-          k = atomicAdd(&s_knext[m], 1u);
-          const uint32_t lim = min(c_Nd, v_rejmin[m]);
-          if (k < lim) { att = 0; have = true; break; }
-          // this move has no unclaimed work left: retire its bit and attach to an unfinished move of the tile
-          atomicAnd(&s_todo[j >> 5], ~(1u << (j & 31)));
-          int found = -1;
+      for (;;) {
+        // ---- claim (divergent, short): lanes without an item take the next k of their move, or re-attach
+        if (active && !have) {
 #pragma unroll 1
-          for (int i = 0; i < NW; ++i) {
-            const int wi = ((j >> 5) + i) % NW;
-            const uint32_t w = v_todo[wi];
-            if (w) {
-              const int r = t & 31;
-              const uint32_t w2 = __funnelshift_r(w, w, r);
-              found = wi * 32 + ((__ffs(w2) - 1 + r) & 31);
-              break;
+          for (;;) {
+            k = atomicAdd(&s_knext[m], 1u);
+            if (k < min(c_Nd, v_rejmin[m])) { att = 0; have = true; break; }
+            // this move has no unclaimed work left: retire its bit, attach to an unfinished move of the tile
+            atomicAnd(&s_todo[j >> 5], ~(1u << (j & 31)));
+            int found = -1;
+#pragma unroll 1
+            for (int i = 0; i < NW; ++i) {
+              const int wi = ((j >> 5) + i) % NW;
+              const uint32_t w = v_todo[wi];
+              if (w) {
+                const int r = t & 31;
+                const uint32_t w2 = __funnelshift_r(w, w, r);
+                found = wi * 32 + ((__ffs(w2) - 1 + r) & 31);
+                break;
+              }
+            }
+            if (found < 0) { active = false; break; }
+            j = found;
+            m = s_alive[j];
+            c_pid = __float_as_uint(s_r1[m].w); c_Nd = s_Nd[m]; c_head = s_head[m]; c_rho = s_rho[m];
+            if (ANISO) {
+              const float4 ao = s_aold[m], an = s_anew[m];
+              c_aold = V3{ao.x, ao.y, ao.z}; c_anew = V3{an.x, an.y, an.z};
             }
           }
-          if (found < 0) { active = false; break; }
-          j = found;
-          m = s_alive[j];
-          c_pid = s_pid[m]; c_Nd = s_Nd[m]; c_head = s_head[m]; c_rho = s_rho[m];
-          if (ANISO) {
-            const float4 ao = s_aold[m], an = s_anew[m];
-            c_aold = V3{ao.x, ao.y, ao.z}; c_anew = V3{an.x, an.y, an.z};
-          }
         }
-        if (!active) break;
-        // one Philox block = one cube-rejection attempt of depletant k (R-S3)
-        const Block4 r = philox(A.key, c_pid, k, 0, c3dep + (att << 16));
-        ++n_blocks;
-        V3 d = V3{g.Rins * sym_unit_bits(r.x), g.Rins * sym_unit_bits(r.y), g.Rins * sym_unit_bits(r.z)};
-        bool inside = dot3(d, d) <= g.Rins2;
-        if (!inside && att == 63u) { d = V3{0.f, 0.f, 0.f}; inside = true; }
-        if (inside) {
-          ++n_eval;
-          const V3 ro = V3{c_rho.x, c_rho.y, c_rho.z};
-          if (q_new_only<SHAPE>(g, d, ro, c_aold, c_anew) && q_free_of_nbrs<SHAPE>(g, s_pool, c_head, d))
-            atomicMin(&s_rejmin[m], k);
-          have = false;
-        } else {
-          ++att;
-          if (k > v_rejmin[m]) have = false;       // a lower k already rejects: this one cannot matter
+        // the vote is also the reconvergence point: the Philox block below runs with the whole warp together
+        if (!__any_sync(0xffffffffu, active)) break;
+        if (active) {
+          // one Philox block = one cube-rejection attempt of depletant k (R-S3)
+          const Block4 r = philox(A.key, c_pid, k, 0, c3dep + (att << 16));
+          ++n_blocks;
+          V3 d = V3{g.Rins * sym_unit_bits(r.x), g.Rins * sym_unit_bits(r.y), g.Rins * sym_unit_bits(r.z)};
+          bool inside = dot3(d, d) <= g.Rins2;
+          if (!inside && att == 63u) { d = V3{0.f, 0.f, 0.f}; inside = true; }
+          if (inside) {
+            ++n_eval;
+            const V3 ro = V3{c_rho.x, c_rho.y, c_rho.z};
+            if (q_new_only<SHAPE>(g, d, ro, c_aold, c_anew) && q_free_of_nbrs<SHAPE>(g, s_pool, c_head, d))
+              atomicMin(&s_rejmin[m], k);
+            have = false;
+          } else {
+            ++att;
+            if (k > v_rejmin[m]) have = false;     // a lower k already rejects: this one cannot matter
+          }
         }
       }
     }
     __syncthreads();
     // ================================================================ commit (a10)
-    if (out != -1) {
-      if (staged) {
-        const uint32_t rm_ = s_rejmin[t];
+#pragma unroll 1
+    for (int e = t; e < nlist; e += T) {
+      int out = (int)s_state[e];
+      const float4 r1f = s_r1[e];
+      const uint32_t pid = __float_as_uint(r1f.w);
+      const bool rot = (s_cell[e] >> 30) & 1u;
+      if (out == OUT_NONE) {
+        const uint32_t Nd = s_Nd[e], rm_ = s_rejmin[e];
         const bool rej = rm_ < Nd;
         out = rej ? OUT_DEPLETANT : OUT_ACCEPT;
         n_drawn += Nd;
@@ -343,18 +379,18 @@ __global__ void __launch_bounds__(T) k_moveq(const QArgs Q) {
       }
       A.outcome[pid] = (uint8_t)out;
       if (out == OUT_ACCEPT) {
+        const uint32_t slot = __float_as_uint(s_rho[e].w);
         float4 pn = A.pos[pid];
-        pn.x = r1.x; pn.y = r1.y; pn.z = r1.z;
+        pn.x = r1f.x; pn.y = r1f.y; pn.z = r1f.z;
         A.pos[pid] = pn;
-        A.cpos[slot] = make_float4(r1.x, r1.y, r1.z, pw);
+        A.cpos[slot] = r1f;
         if (ANISO && rot) {
-          A.quat[pid] = as_f4(q1);
-          const V3 an = quat_axis(q1);
+          A.quat[pid] = s_q1[e];
+          const float4 an = s_anew[e];
           A.caxis[slot] = make_float4(an.x, an.y, an.z, 0.0f);
         }
         if (rot) ++n_ar; else ++n_at;
-      } else if (out == OUT_BOUNDARY) ++n_rb;
-      else if (out == OUT_HARD) ++n_rh;
+      } else if (out == OUT_HARD) ++n_rh;
       else ++n_rd;
     }
     __syncthreads();
