@@ -106,6 +106,8 @@ class HPMC:
                 assert quat4.is_cuda and quat4.dtype == torch.float32 and quat4.is_contiguous() and quat4.shape == pos4.shape
         self.N = int(N)
         self.pos4, self.quat4 = pos4, quat4           # keep the borrowed tensors alive
+        if stream is None and not torch.cuda.is_available():
+            raise HPMCError(-5, "no CUDA device: this library has no CPU path")
         s = torch.cuda.current_stream() if stream is None else stream
         self.stream = s
         h = C.c_void_p()
