@@ -31,8 +31,12 @@ import workloads  # noqa: E402
 # Algorithmic work per unit: lane-operations (one thread executing one plain ALU instruction).
 OPS_PER_NEEDED_DEPLETANT = 131.0   # 1.91 attempts x (40 INT Philox + 22 convert/scale/|d|^2/compare) + 11 pose tests + ~2 nbr
 OPS_PER_MOVE = 500.0               # 3 Philox blocks, 27-cell staging, hard overlap, table search, commit
-BYTES_PER_MOVE = 470.0             # cell_start words + 27<occ> staged float4
+BYTES_PER_PARTICLE_PER_PASS = 16.0 # every pass reads the cell-ordered float4 array once (re-reads by neighbouring cells are L2 hits)
+BYTES_PER_CELL_PER_PASS = 4.0      # ... and each cell_start word once
+BYTES_PER_MOVE = 1.0               # outcome code
 BYTES_PER_ACCEPT = 48.0
+# dram__bytes_read.sum + dram__bytes_write.sum of one move-kernel launch at C3, ncu --set full (profiles/r1b_summary.md)
+NCU_TRAFFIC_BYTES_PER_LAUNCH_C3 = 22.43e6
 LANES_PER_SM_PER_CLK = 128.0       # 4 SMSPs x 32 lanes: issue-rate peak of the plain ALU pipes
 NUM_SMS = 148
 
@@ -102,6 +106,19 @@ class ClockSampler:
         if sm:
             out = {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons), "samples": len(sm)}
         return out
+
+
+def reduce_over_ranks(total_ms, work, device, world):
+    """Replicas only: the job's time is the MAX over ranks of the timed duration, its work the SUM over
+    ranks.  The one place bench.py talks to torch.distributed besides the barrier; covered by a gloo test on CPU."""
+    import torch
+    t = torch.tensor([total_ms], dtype=torch.float64, device=device)
+    w = torch.tensor(list(work), dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(w, op=dist.ReduceOp.SUM)
+    return float(t.item()), [float(x) for x in w.tolist()]
 
 
 def oracle_sample(cfg, pos, quat, sweeps, step0):
@@ -225,13 +242,9 @@ def main():
     moves = c["trials_trans"] + c["trials_rot"]
 
     # max over ranks of the timed duration, sum over ranks of the work
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    w = torch.tensor([moves, c["dep_evaluated"], c["dep_needed"], c["dep_drawn"]], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(w, op=dist.ReduceOp.SUM)
-    tot_s = float(t.item()) * 1e-3
-    g_moves, g_eval, g_needed, g_drawn = [float(x) for x in w.tolist()]
+    job_ms, (g_moves, g_eval, g_needed, g_drawn) = reduce_over_ranks(
+        total_ms, [moves, c["dep_evaluated"], c["dep_needed"], c["dep_drawn"]], "cuda", world)
+    tot_s = job_ms * 1e-3
 
     # ---- e2e: the same step through the host-buffer C-ABI call, copies inside the timed region
     e2e = None
@@ -251,20 +264,17 @@ def main():
         e1.record()
         barrier()
         ce = hh.counters()
-        te = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
-        we = torch.tensor([ce["trials_trans"] + ce["trials_rot"]], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-            dist.all_reduce(we, op=dist.ReduceOp.SUM)
+        te, (we,) = reduce_over_ranks(e0.elapsed_time(e1), [ce["trials_trans"] + ce["trials_rot"]], "cuda", world)
         nq = 2 if quat is not None else 1
-        e2e = {"value": float(we.item()) / (float(te.item()) * 1e-3), "unit": "moves/s",
+        e2e = {"value": we / (te * 1e-3), "unit": "moves/s",
                "h2d_bytes_per_step": 16 * cfg.N * nq, "d2h_bytes_per_step": 16 * cfg.N * nq + cfg.N,
-               "ms_per_step": float(te.item()) / args.steps}
+               "ms_per_step": te / args.steps}
         hh.close()
 
     if rank == 0:
         alg_ops = c["dep_needed"] * OPS_PER_NEEDED_DEPLETANT + moves * OPS_PER_MOVE
-        alg_bytes = moves * BYTES_PER_MOVE + (c["accept_trans"] + c["accept_rot"]) * BYTES_PER_ACCEPT
+        alg_bytes = (move_launches * (BYTES_PER_PARTICLE_PER_PASS * cfg.N + BYTES_PER_CELL_PER_PASS * (h.n_c ** 3 + 1))
+                     + moves * BYTES_PER_MOVE + (c["accept_trans"] + c["accept_rot"]) * BYTES_PER_ACCEPT)
         move_s = move_ms * 1e-3
         alu_peak = NUM_SMS * LANES_PER_SM_PER_CLK * pk["sm_max_mhz"] * 1e6          # lane-ops/s at max boost clock
         alu_ach = alg_ops / move_s if move_s > 0 else 0.0
@@ -273,7 +283,9 @@ def main():
         roofline = {
             "bound": "alu" if t_alu >= t_hbm else "hbm",
             "achieved": alu_ach / 1e12, "peak": alu_peak / 1e12, "unit": "Tlaneop/s", "frac": alu_ach / alu_peak,
-            "traffic": None, "kernel": "k_move", "launches": move_launches,
+            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH_C3 if (cfg.name == "C3" and args.n is None) else None,
+            "alg_bytes_per_launch": alg_bytes / max(1, move_launches), "alg_laneops_per_launch": alg_ops / max(1, move_launches),
+            "kernel": "k_moveq (8 launches per step)", "launches": move_launches,
             "avg_launch_ms": move_ms / max(1, move_launches), "share_of_step": move_ms / total_ms if total_ms else None,
             "peak_source": "derived: 148 SM x 128 lanes/clk x %.0f MHz (DESIGN.md); HBM %s" % (pk["sm_max_mhz"], pk["source"]),
             "hbm": {"achieved": hbm_ach, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": hbm_ach / pk["hbm_gbs"]},
@@ -289,7 +301,7 @@ def main():
                    "dep_needed_per_s": oc["dep_needed"] / sum(times)}
         line = {
             "metric": "colloid_trial_moves_per_s", "value": g_moves / tot_s, "unit": "moves/s", "n_gpus": world,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": float(t.item()) / args.steps,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": job_ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_desc(cfg), "step": "one sweep = cell build + 8 checkerboard passes",
                        "l2": "flushed between timed steps (512 MiB write)", "parallelism": "replicas x%d" % world,
