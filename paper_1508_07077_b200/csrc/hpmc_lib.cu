@@ -31,6 +31,8 @@ struct PoissonTable {
   uint32_t k_lo = 0;
   int n = 0;
   unsigned long long* d_T = nullptr;
+  uint16_t* d_G = nullptr;              // guide table (1025 entries) or nullptr when the table has > 65535 entries
+  bool has_guide = false;
   size_t cap = 0;
 };
 
@@ -63,7 +65,8 @@ struct hpmc_ctx {
   int num_sms = 148;
   int move_ctas = 0;
   unsigned int* d_tiles = nullptr;     // 8 tile counters, one per pass of a sweep
-  int q_ctas = 0;                      // persistent CTAs of the item-queue move kernel
+  int q_ctas = 0;                      // CTAs of the item-queue move kernel
+  int q_tile_cells = 0;                // active cells per tile (one wave)
   bool use_queue = true;               // HPMC_MOVE_KERNEL=warp selects the first (warp-per-cell) design
   int64_t launches = 0;
   bool timing = false;
@@ -150,9 +153,24 @@ int get_table(hpmc_ctx* ctx, double lambda, PoissonTable** out) {
     slot->cap = T.size() + 64;
     CU(cudaMalloc(&slot->d_T, slot->cap * sizeof(unsigned long long)));
   }
+  slot->has_guide = false;
   if (!T.empty()) {
     // pageable source: the runtime stages it before returning, so T may go out of scope
     CU(cudaMemcpyAsync(slot->d_T, T.data(), T.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice, ctx->stream));
+    if (T.size() <= 65535) {
+      // guide table: G[i] = #{j : T[j] < i 2^54}; the count for a uniform U with top bits b lies in [G[b], G[b+1]]
+      std::vector<uint16_t> G(1025);
+      size_t j = 0;
+      for (unsigned i = 0; i < 1024; ++i) {
+        const unsigned long long edge = (unsigned long long)i << 54;
+        while (j < T.size() && T[j] < edge) ++j;
+        G[i] = (uint16_t)j;
+      }
+      G[1024] = (uint16_t)T.size();
+      if (!slot->d_G) CU(cudaMalloc(&slot->d_G, 1025 * sizeof(uint16_t)));
+      CU(cudaMemcpyAsync(slot->d_G, G.data(), 1025 * sizeof(uint16_t), cudaMemcpyHostToDevice, ctx->stream));
+      slot->has_guide = true;
+    }
     CU(cudaStreamSynchronize(ctx->stream));
   }
   slot->lambda = lambda; slot->k_lo = klo; slot->n = (int)T.size();
@@ -161,37 +179,47 @@ int get_table(hpmc_ctx* ctx, double lambda, PoissonTable** out) {
 }
 
 constexpr int QT = 128;                // threads per CTA of the item-queue kernel
-constexpr int QCPT = 2;                // active cells per thread and tile
 
 template <int SHAPE>
 int setup_moveq(hpmc_ctx* ctx) {
-  const size_t smem = QSmem<SHAPE, QT, QCPT>::bytes;
-  cudaError_t e = cudaFuncSetAttribute(k_moveq<SHAPE, QT, QCPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  const size_t smem = QSmem<SHAPE, QT>::bytes;
+  cudaError_t e = cudaFuncSetAttribute(k_moveq<SHAPE, QT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return fail(ctx, HPMC_E_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
   int per_sm = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_moveq<SHAPE, QT, QCPT>, QT, smem);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_moveq<SHAPE, QT>, QT, smem);
   if (e != cudaSuccess || per_sm < 1) return fail(ctx, HPMC_E_CUDA, "k_moveq does not fit on an SM");
-  const int ntiles = (ctx->ncell / 8 + QT * QCPT - 1) / (QT * QCPT);
-  int ctas = ctx->num_sms * per_sm;
-  if (ctas > ntiles) ctas = ntiles;
-  ctx->q_ctas = ctas < 1 ? 1 : ctas;
+  // one wave: tiles sized so that every tile of a pass is resident at once (a pass is latency-, not throughput-bound)
+  const int nact = ctx->ncell / 8;
+  const int resident = ctx->num_sms * per_sm;
+  const long long waves = ((long long)nact + (long long)resident * QT - 1) / ((long long)resident * QT);
+  int tc = (int)((nact + waves * resident - 1) / (waves * resident));   // every CTA gets `waves` tiles of equal size
+  if (tc < 16) tc = 16;
+  if (tc > QT) tc = QT;
+  if (const char* o = getenv("HPMC_TILE_CELLS")) { const int v = atoi(o); if (v >= 1 && v <= QT) tc = v; }
+  ctx->q_tile_cells = tc;
+  const int ntiles = (nact + tc - 1) / tc;
+  ctx->q_ctas = ntiles < resident ? ntiles : resident;
+  if (getenv("HPMC_VERBOSE"))
+    fprintf(stderr, "k_moveq<%d,%d>: smem %zu B, %d CTAs/SM, tile %d cells, %d tiles, %d CTAs\n", SHAPE, QT, smem, per_sm, tc,
+            ntiles, ctx->q_ctas);
   return 0;
 }
 
 template <int SHAPE>
-int launch_moveq(hpmc_ctx* ctx, const MoveArgs& a, int pass) {
+int launch_moveq(hpmc_ctx* ctx, const MoveArgs& a, const PoissonTable* pt) {
   QArgs q;
   q.m = a;
   q.magic_hc = ~0ull / (unsigned long long)a.hc + 1ull;   // floor((2^64-1)/hc)+1 == floor(2^64/hc)+1 unless hc | 2^64
   if ((a.hc & (a.hc - 1)) == 0) q.magic_hc = (1ull << 63) / (unsigned long long)a.hc * 2ull + 1ull;
-  q.tile_counter = ctx->d_tiles + pass;
-  q.ntiles = (a.nact + QT * QCPT - 1) / (QT * QCPT);
+  q.pguide = pt->has_guide ? pt->d_G : nullptr;
+  q.tile_cells = ctx->q_tile_cells;
+  q.ntiles = (a.nact + q.tile_cells - 1) / q.tile_cells;
   {
     const float rl = (ctx->p.sigma_c + ctx->p.sigma_d) + 1e-3f;
     q.rlist2 = rl * rl;
     if (q.rlist2 > a.g.rcut2) q.rlist2 = a.g.rcut2;
   }
-  k_moveq<SHAPE, QT, QCPT><<<ctx->q_ctas, QT, QSmem<SHAPE, QT, QCPT>::bytes, ctx->stream>>>(q);
+  k_moveq<SHAPE, QT><<<ctx->q_ctas, QT, QSmem<SHAPE, QT>::bytes, ctx->stream>>>(q);
   return 0;
 }
 
@@ -288,7 +316,7 @@ void hpmc_destroy(hpmc_ctx* ctx) {
   cudaFree(ctx->d_cpos); cudaFree(ctx->d_caxis); cudaFree(ctx->d_cid); cudaFree(ctx->d_rank);
   cudaFree(ctx->d_cell_pid); cudaFree(ctx->d_counts); cudaFree(ctx->d_cell_start); cudaFree(ctx->d_tile_sums);
   cudaFree(ctx->d_outcome); cudaFree(ctx->d_counters); cudaFree(ctx->d_err); cudaFree(ctx->d_tiles);
-  for (auto& t : ctx->tables) cudaFree(t.d_T);
+  for (auto& t : ctx->tables) { cudaFree(t.d_T); cudaFree(t.d_G); }
   for (auto& e : ctx->ev) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   delete ctx;
 }
@@ -346,7 +374,6 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
     const uint32_t t = perm[i]; perm[i] = perm[r]; perm[r] = t;
   }
   CU(cudaMemsetAsync(ctx->d_outcome, 0, (size_t)ctx->N, ctx->stream));
-  CU(cudaMemsetAsync(ctx->d_tiles, 0, sizeof(unsigned int) * 8, ctx->stream));
 
   MoveArgs a;
   a.g = ctx->g; a.key = key;
@@ -372,9 +399,9 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
     }
     if (ctx->use_queue && !cb) {
       switch (ctx->p.shape) {
-        case HPMC_SPHERE: launch_moveq<SH_SPHERE>(ctx, a, pass); break;
-        case HPMC_HALFBALL: launch_moveq<SH_HALFBALL>(ctx, a, pass); break;
-        default: launch_moveq<SH_SPHERODISK>(ctx, a, pass); break;
+        case HPMC_SPHERE: launch_moveq<SH_SPHERE>(ctx, a, pt); break;
+        case HPMC_HALFBALL: launch_moveq<SH_HALFBALL>(ctx, a, pt); break;
+        default: launch_moveq<SH_SPHERODISK>(ctx, a, pt); break;
       }
     } else {
       switch (ctx->p.shape) {

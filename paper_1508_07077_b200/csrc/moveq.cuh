@@ -1,14 +1,20 @@
-// moveq.cuh -- steps a3..a10, second design of the checkerboard move kernel (K-B): "thread per cell + item queue".
+// moveq.cuh -- steps a3..a10, item-queue design of the checkerboard move kernel (K-B).
 //
-// A CTA of T threads takes tiles of CPT*T active cells (dynamic tile counter, persistent CTAs).
-//   phase 1a one THREAD per active cell (CPT cells each): pick (a3), trial pose + confinement (a4).  Moves that
-//            stay in their cell are compacted into a dense list in shared memory (empty cells and boundary
-//            rejections -- about half of the cells at C3 -- drop out here).
-//   phase 1b one thread per listed move: one walk over the 27-cell neighbourhood (a5) with the sphere
-//            hard-overlap test inline (a6), then N_d by table inversion (a7).  Neighbours that a depletant of
-//            this move can touch go to a per-move linked list in a CTA-wide shared-memory pool.
-//   phase 1c (convex shapes) the (move, neighbour) pairs inside the circumsphere distance become items; the
-//            CTA's lanes run the support-function test on them side by side.
+// C3 has 175,616 active cells per pass and a B200 holds ~300k resident threads, so a pass is ONE wave of work: its
+// duration is the serial latency chain of a tile, not a throughput.  The kernel is therefore organised to keep every
+// chain short and every phase spread over all T lanes of the CTA:
+//   tiling   tiles of `tile_cells` <= T active cells, sized by the host so that all tiles are resident at once
+//            (one wave, static assignment tile = blockIdx.x + i gridDim.x: no tile counter, no second-tile tail).
+//   phase 1a one THREAD per active cell: pick (a3), trial pose + confinement (a4).  Moves that stay in their cell are
+//            compacted into a dense list in shared memory (empty cells and boundary rejections drop out here).
+//   phase 1b one thread per (move, x-row) item, 9 rows per move: the row's 3 cells are one contiguous span of the
+//            cell-ordered array (two spans when the row wraps); particles are loaded four at a time, the sphere
+//            hard-overlap test runs inline (a5, a6), neighbours that a depletant of the move can touch are pushed on
+//            the move's linked list in a CTA-wide shared-memory pool.
+//   phase 1c (convex shapes) the (move, neighbour) pairs inside the circumsphere distance are items of their own;
+//            the CTA's lanes run the support-function test on them side by side.
+//   phase 1d one thread per move: N_d by table inversion (a7), three dependent loads instead of eleven thanks to a
+//            1024-bucket guide table indexed by the top 10 bits of the uniform.
 //   phase 2  the depletant insertions of ALL surviving moves of the tile are one pool of items
 //            (move m, depletant k, attempt a).  Every lane repeatedly claims the next k of the move it is
 //            attached to (shared-memory atomic), computes ONE Philox block per loop trip, and on an accepted
@@ -19,7 +25,8 @@
 //   commit   the owner thread writes outcome, pose, counters (a10).
 // Results are identical to the sequential definition: the outcome depends only on whether a rejecting depletant
 // exists, and dep_needed = (smallest rejecting k) + 1 is exact because k's are claimed in ascending order and a
-// claimed k below the current minimum is never abandoned.
+// claimed k below the current minimum is never abandoned.  The order of a move's neighbour list does not matter:
+// "overlaps no other colloid" is a disjunction.
 //
 // PAPER.md: move rule L64-68, Fig. 2 L72; insertion sphere L156; checkerboard + confinement L180; the paper's
 // own GPU layout (App. A: one kernel for trial moves, one thread GROUP per depletant) is prior art.
@@ -34,7 +41,8 @@ namespace hpmc {
 struct QArgs {
   MoveArgs m;
   unsigned long long magic_hc;     // floor(2^64 / hc) + 1: exact a / hc by __umul64hi for a < 2^32
-  unsigned int* tile_counter;      // one word per pass, zeroed by the host before the sweep
+  const uint16_t* pguide;          // [1025] G[i] = #{j : T[j] < i 2^54}, or nullptr (plain binary search)
+  int tile_cells;                  // active cells per tile, <= T
   int ntiles;
   float rlist2;                    // neighbours farther than this from the new centre cannot touch any depletant
                                    // of the move: (sigma_c + sigma_d + 1e-3)^2 for the plain rule (insertion
@@ -52,17 +60,17 @@ template <int SHAPE>
 struct QLayout {
   static constexpr bool ANISO = SHAPE != SH_SPHERE;
   static constexpr int ENTRY = ANISO ? 2 : 1;                 // float4 per neighbour entry
-  static constexpr int POOL_PER_THREAD = ANISO ? 12 : 8;      // pool capacity = this x T entries
-  static constexpr int HCAP_PER_THREAD = 4;                   // hard-test items (convex shapes) = this x T
+  static constexpr int POOL_PER_MOVE = ANISO ? 12 : 6;        // pool capacity = this x T entries (tile average)
+  static constexpr int HCAP_PER_MOVE = 4;                     // hard-test items (convex shapes) = this x T
 };
 
-// shared-memory carve-up for a CTA of T threads handling M = CPT*T cells per tile
-template <int SHAPE, int T, int CPT>
+// shared-memory carve-up for a CTA of T threads handling up to M = T moves per tile
+template <int SHAPE, int T>
 struct QSmem {
   using Lq = QLayout<SHAPE>;
-  static constexpr int M = CPT * T;
-  static constexpr int POOL = Lq::POOL_PER_THREAD * T;
-  static constexpr int HCAP = Lq::ANISO ? Lq::HCAP_PER_THREAD * T : 0;
+  static constexpr int M = T;
+  static constexpr int POOL = Lq::POOL_PER_MOVE * T;
+  static constexpr int HCAP = Lq::ANISO ? Lq::HCAP_PER_MOVE * T : 0;
   static constexpr size_t o_r1 = 0;                                             // float4[M]  r1.xyz, pid bits
   static constexpr size_t o_rho = o_r1 + sizeof(float4) * M;                    // float4[M]  rho_old.xyz, slot bits
   static constexpr size_t o_q1 = o_rho + sizeof(float4) * M;                    // float4[M]  new quaternion (aniso)
@@ -100,10 +108,25 @@ __device__ __forceinline__ bool q_free_of_nbrs(const Geo& g, const float4* pool,
   return true;
 }
 
-template <int SHAPE, int T, int CPT>
+// N_d = k_lo + #{j : T[j] <= U} (R-S2).  With the guide table the search starts from the bucket of U's top 10 bits.
+__device__ __forceinline__ uint32_t poisson_count(const unsigned long long* __restrict__ T, int n,
+                                                  const uint16_t* __restrict__ guide, unsigned long long U) {
+  int lo = 0, hi = n;
+  if (guide) {
+    const uint32_t b = (uint32_t)(U >> 54);
+    lo = __ldg(&guide[b]); hi = __ldg(&guide[b + 1]);
+  }
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (__ldg(&T[mid]) <= U) lo = mid + 1; else hi = mid;
+  }
+  return (uint32_t)lo;
+}
+
+template <int SHAPE, int T>
 __global__ void __launch_bounds__(T) k_moveq(const QArgs Q) {
   using Lq = QLayout<SHAPE>;
-  using S = QSmem<SHAPE, T, CPT>;
+  using S = QSmem<SHAPE, T>;
   constexpr bool ANISO = Lq::ANISO;
   constexpr int E = Lq::ENTRY;
   constexpr int M = S::M, POOL = S::POOL, HCAP = S::HCAP, NW = M / 32;
@@ -126,7 +149,7 @@ __global__ void __launch_bounds__(T) k_moveq(const QArgs Q) {
   uint32_t* s_state = reinterpret_cast<uint32_t*>(sb_ + S::o_state);
   uint32_t* s_todo = reinterpret_cast<uint32_t*>(sb_ + S::o_todo);
   uint32_t* s_hitems = reinterpret_cast<uint32_t*>(sb_ + S::o_hitems);
-  uint32_t* s_scal = reinterpret_cast<uint32_t*>(sb_ + S::o_scal);   // [0] nalive [1] pool top [2] tile [3] nhard [4] nlist
+  uint32_t* s_scal = reinterpret_cast<uint32_t*>(sb_ + S::o_scal);   // [0] nalive [1] pool top [3] nhard [4] nlist
   uint16_t* s_alive = reinterpret_cast<uint16_t*>(sb_ + S::o_alive);
 
   const int t = threadIdx.x;
@@ -139,152 +162,152 @@ __global__ void __launch_bounds__(T) k_moveq(const QArgs Q) {
   uint32_t n_tt = 0, n_at = 0, n_tr = 0, n_ar = 0, n_rb = 0, n_rh = 0, n_rd = 0;
   uint32_t n_drawn = 0, n_needed = 0, n_eval = 0, n_blocks = 0;
 
-  for (;;) {
-    if (t == 0) {
-      s_scal[2] = atomicAdd(Q.tile_counter, 1u);
-      s_scal[0] = 0; s_scal[1] = 0; s_scal[3] = 0; s_scal[4] = 0;
-    }
+  for (uint32_t tile = blockIdx.x; tile < (uint32_t)Q.ntiles; tile += gridDim.x) {
+    if (t == 0) { s_scal[0] = 0; s_scal[1] = 0; s_scal[3] = 0; s_scal[4] = 0; }
     __syncthreads();
-    const uint32_t tile = s_scal[2];
-    if (tile >= (uint32_t)Q.ntiles) break;
 
     // ================================================================ phase 1a: one thread per active cell
-#pragma unroll 1
-    for (int c = 0; c < CPT; ++c) {
-      const uint32_t a = tile * M + c * T + t;
-      if (a >= (uint32_t)A.nact) continue;
-      const uint32_t q1d = (uint32_t)__umul64hi((unsigned long long)a, Q.magic_hc);        // a / hc
-      const uint32_t q2d = (uint32_t)__umul64hi((unsigned long long)q1d, Q.magic_hc);      // a / hc^2
-      const int ix = 2 * (int)(a - q1d * hc) + px, iy = 2 * (int)(q1d - q2d * hc) + py, iz = 2 * (int)q2d + pz;
-      const uint32_t cell = ((uint32_t)iz * nc + iy) * nc + ix;
-      const uint32_t cb = A.cell_start[cell], ce = A.cell_start[cell + 1];
-      const uint32_t nocc = ce - cb;
-      if (nocc == 0) continue;
-      // ---- a3: pick
-      const Block4 rs = philox(A.key, cell, 0, 0, P_SELECT + colw);
-      const uint32_t slot = cb + __umulhi(rs.x, nocc);
-      const float4 p0 = A.cpos[slot];
-      const uint32_t pid = __float_as_uint(p0.w);
-      const V3 r0 = V3{p0.x, p0.y, p0.z};
-      Q4 q0 = Q4{1.0f, 0.0f, 0.0f, 0.0f};
-      if (ANISO) q0 = as_q(A.quat[pid]);
-      // ---- a4: trial pose
-      const Block4 rm = philox(A.key, pid, 0, 0, P_MOVE + colw);
-      n_blocks += 2;
-      const bool rot = (A.a_max > 0.0f) && (rm.w & 1u);
-      V3 r1 = r0;
-      Q4 q1 = q0;
-      if (!rot) {
-        r1 = V3{wrap1(g, r0.x + A.d_max * sym_unit_bits(rm.x)), wrap1(g, r0.y + A.d_max * sym_unit_bits(rm.y)),
-                wrap1(g, r0.z + A.d_max * sym_unit_bits(rm.z))};
-        ++n_tt;
-      } else {
-        const V3 v = ball_sample(A.key, pid, 0, 0, P_MOVE + colw + (1u << 16), A.a_max, A.a_max2, n_blocks);
-        q1 = rotate_cayley(q0, v);
-        ++n_tr;
-      }
-      const int jx = cell_axis(g, r1.x, A.sx), jy = cell_axis(g, r1.y, A.sy), jz = cell_axis(g, r1.z, A.sz);
-      if (jx != ix || jy != iy || jz != iz) {        // confinement (L180)
-        A.outcome[pid] = (uint8_t)OUT_BOUNDARY;
-        ++n_rb;
-        continue;
-      }
-      const uint32_t e = atomicAdd(&s_scal[4], 1u);
-      s_r1[e] = make_float4(r1.x, r1.y, r1.z, p0.w);
-      s_rho[e] = make_float4(minimg1(g, r0.x - r1.x), minimg1(g, r0.y - r1.y), minimg1(g, r0.z - r1.z),
-                             __uint_as_float(slot));
-      s_cell[e] = (uint32_t)ix | ((uint32_t)iy << 10) | ((uint32_t)iz << 20) | (rot ? (1u << 30) : 0u);
-      if (ANISO) {
-        s_q1[e] = as_f4(q1);
-        const V3 ao = quat_axis(q0), an = quat_axis(q1);
-        s_aold[e] = make_float4(ao.x, ao.y, ao.z, 0.0f);
-        s_anew[e] = make_float4(an.x, an.y, an.z, 0.0f);
+    if (t < Q.tile_cells) {
+      const uint32_t a = tile * (uint32_t)Q.tile_cells + (uint32_t)t;
+      if (a < (uint32_t)A.nact) {
+        const uint32_t q1d = (uint32_t)__umul64hi((unsigned long long)a, Q.magic_hc);        // a / hc
+        const uint32_t q2d = (uint32_t)__umul64hi((unsigned long long)q1d, Q.magic_hc);      // a / hc^2
+        const int ix = 2 * (int)(a - q1d * hc) + px, iy = 2 * (int)(q1d - q2d * hc) + py, iz = 2 * (int)q2d + pz;
+        const uint32_t cell = ((uint32_t)iz * nc + iy) * nc + ix;
+        const uint32_t cb = A.cell_start[cell], ce = A.cell_start[cell + 1];
+        const uint32_t nocc = ce - cb;
+        if (nocc != 0) {
+          // ---- a3: pick
+          const Block4 rs = philox(A.key, cell, 0, 0, P_SELECT + colw);
+          const uint32_t slot = cb + __umulhi(rs.x, nocc);
+          const float4 p0 = A.cpos[slot];
+          const uint32_t pid = __float_as_uint(p0.w);
+          const V3 r0 = V3{p0.x, p0.y, p0.z};
+          Q4 q0 = Q4{1.0f, 0.0f, 0.0f, 0.0f};
+          if (ANISO) q0 = as_q(A.quat[pid]);
+          // ---- a4: trial pose
+          const Block4 rm = philox(A.key, pid, 0, 0, P_MOVE + colw);
+          n_blocks += 2;
+          const bool rot = (A.a_max > 0.0f) && (rm.w & 1u);
+          V3 r1 = r0;
+          Q4 q1 = q0;
+          if (!rot) {
+            r1 = V3{wrap1(g, r0.x + A.d_max * sym_unit_bits(rm.x)), wrap1(g, r0.y + A.d_max * sym_unit_bits(rm.y)),
+                    wrap1(g, r0.z + A.d_max * sym_unit_bits(rm.z))};
+            ++n_tt;
+          } else {
+            const V3 v = ball_sample(A.key, pid, 0, 0, P_MOVE + colw + (1u << 16), A.a_max, A.a_max2, n_blocks);
+            q1 = rotate_cayley(q0, v);
+            ++n_tr;
+          }
+          const int jx = cell_axis(g, r1.x, A.sx), jy = cell_axis(g, r1.y, A.sy), jz = cell_axis(g, r1.z, A.sz);
+          if (jx != ix || jy != iy || jz != iz) {        // confinement (L180)
+            A.outcome[pid] = (uint8_t)OUT_BOUNDARY;
+            ++n_rb;
+          } else {
+            const uint32_t e = atomicAdd(&s_scal[4], 1u);
+            s_r1[e] = make_float4(r1.x, r1.y, r1.z, p0.w);
+            s_rho[e] = make_float4(minimg1(g, r0.x - r1.x), minimg1(g, r0.y - r1.y), minimg1(g, r0.z - r1.z),
+                                   __uint_as_float(slot));
+            s_cell[e] = (uint32_t)ix | ((uint32_t)iy << 10) | ((uint32_t)iz << 20) | (rot ? (1u << 30) : 0u);
+            s_head[e] = -1;
+            s_state[e] = OUT_NONE;
+            if (ANISO) {
+              s_q1[e] = as_f4(q1);
+              const V3 ao = quat_axis(q0), an = quat_axis(q1);
+              s_aold[e] = make_float4(ao.x, ao.y, ao.z, 0.0f);
+              s_anew[e] = make_float4(an.x, an.y, an.z, 0.0f);
+            }
+          }
+        }
       }
     }
     __syncthreads();
     const int nlist = (int)s_scal[4];
 
-    // ================================================================ phase 1b: one thread per listed move
+    // ================================================================ phase 1b: one thread per (move, x-row) item
 #pragma unroll 1
-    for (int e = t; e < nlist; e += T) {
+    for (int it = t; it < nlist * 9; it += T) {
+      const int e = it / 9, row = it - 9 * e;
       const float4 r1f = s_r1[e];
       const V3 r1 = V3{r1f.x, r1f.y, r1f.z};
-      const uint32_t pid = __float_as_uint(r1f.w);
       const uint32_t slot = __float_as_uint(s_rho[e].w);
       const uint32_t cw = s_cell[e];
       const int ix = cw & 1023, iy = (cw >> 10) & 1023, iz = (cw >> 20) & 1023;
-      V3 a_new = V3{0.f, 0.f, 1.f};
-      if (ANISO) { const float4 an = s_anew[e]; a_new = V3{an.x, an.y, an.z}; }
-      // ---- a5 + a6: one walk over the 27 cells (9 x-rows; a row is one contiguous span unless it wraps)
+      const int dz = row / 3 - 1, dy = row - 3 * (row / 3) - 1;
+      int jy = iy + dy, jz = iz + dz;
+      jy += (jy < 0) ? nc : 0; jy -= (jy >= nc) ? nc : 0;
+      jz += (jz < 0) ? nc : 0; jz -= (jz >= nc) ? nc : 0;
+      const uint32_t rb = ((uint32_t)jz * nc + jy) * nc;
+      // ---- a5: the row's 3 cells are one contiguous span unless the row wraps in x
       int x0 = ix - 1, n0 = 3, n1 = 0;
       if (ix == 0) { x0 = nc - 1; n0 = 1; n1 = 2; }
       else if (ix == nc - 1) { x0 = nc - 2; n0 = 2; n1 = 1; }
-      int head = -1;
-      bool hard = false;
-      for (int row = 0; row < 9 && !hard; ++row) {
-        const int dz = row / 3 - 1, dy = row % 3 - 1;
-        int jy = iy + dy, jz = iz + dz;
-        jy += (jy < 0) ? nc : 0; jy -= (jy >= nc) ? nc : 0;
-        jz += (jz < 0) ? nc : 0; jz -= (jz >= nc) ? nc : 0;
-        const uint32_t rb = ((uint32_t)jz * nc + jy) * nc;
-        for (int seg = 0; seg < 2 && !hard; ++seg) {
-          const int xs = seg ? 0 : x0, nn = seg ? n1 : n0;
-          if (nn == 0) break;
-          const uint32_t sb = A.cell_start[rb + xs], se = A.cell_start[rb + xs + nn];
-          for (uint32_t s = sb; s < se; ++s) {
-            if (s == slot) continue;
-            const float4 pj = A.cpos[s];
-            const V3 rho = V3{minimg1(g, pj.x - r1.x), minimg1(g, pj.y - r1.y), minimg1(g, pj.z - r1.z)};
+#pragma unroll 1
+      for (int seg = 0; seg < 2; ++seg) {
+        const int xs = seg ? 0 : x0, nn = seg ? n1 : n0;
+        if (nn == 0) break;
+        const uint32_t sb = A.cell_start[rb + xs], se = A.cell_start[rb + xs + nn];
+#pragma unroll 1
+        for (uint32_t s0 = sb; s0 < se; s0 += 4) {
+          float4 pj[4];
+#pragma unroll
+          for (int i = 0; i < 4; ++i)
+            if (s0 + i < se) pj[i] = A.cpos[s0 + i];
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const uint32_t s = s0 + i;
+            if (s >= se || s == slot) continue;
+            const V3 rho = V3{minimg1(g, pj[i].x - r1.x), minimg1(g, pj[i].y - r1.y), minimg1(g, pj[i].z - r1.z)};
             const float r2 = dot3(rho, rho);
             if (!(r2 < Q.rlist2)) continue;
-            if (!ANISO && r2 < g.dcirc2) { hard = true; break; }
+            if (!ANISO && r2 < g.dcirc2) { s_state[e] = OUT_HARD; continue; }     // a6 (spheres)
             const int pe = (int)atomicAdd(&s_scal[1], 1u);
             if (pe >= POOL) { atomicExch(A.err_flag, 1); continue; }
-            s_pool[pe * E] = make_float4(rho.x, rho.y, rho.z, __int_as_float(head));
-            head = pe;
+            const int prev = atomicExch(&s_head[e], pe);
+            s_pool[pe * E] = make_float4(rho.x, rho.y, rho.z, __int_as_float(prev));
             if (ANISO) {
               const float4 axj = A.caxis[s];
               s_pool[pe * E + 1] = axj;
               if (r2 < g.dcirc2) {
                 const uint32_t hi = atomicAdd(&s_scal[3], 1u);
                 if (hi < (uint32_t)HCAP) s_hitems[hi] = ((uint32_t)e << 16) | (uint32_t)pe;
-                else if (mpr_overlap<SHAPE>(g, rho, a_new, V3{axj.x, axj.y, axj.z})) hard = true;
+                else {
+                  const float4 an = s_anew[e];
+                  if (mpr_overlap<SHAPE>(g, rho, V3{an.x, an.y, an.z}, V3{axj.x, axj.y, axj.z})) s_state[e] = OUT_HARD;
+                }
               }
             }
           }
         }
       }
-      uint32_t Nd = 0;
-      if (!hard && A.pt_n > 0) {
-        // ---- a7: N_d by table inversion
-        const Block4 rn = philox(A.key, pid, 0, 0, P_NDEP + colw);
-        ++n_blocks;
-        const unsigned long long U = ((unsigned long long)rn.x << 32) | rn.y;
-        int lo = 0, hi = A.pt_n;
-        while (lo < hi) {
-          const int mid = (lo + hi) >> 1;
-          if (__ldg(&A.ptable[mid]) <= U) lo = mid + 1; else hi = mid;
-        }
-        Nd = A.pt_klo + (uint32_t)lo;
-      }
-      s_Nd[e] = Nd; s_knext[e] = 0; s_rejmin[e] = 0xffffffffu; s_head[e] = head;
-      s_state[e] = hard ? OUT_HARD : OUT_NONE;
-      if (!ANISO && !hard && Nd != 0) s_alive[atomicAdd(&s_scal[0], 1u)] = (uint16_t)e;
     }
-    // ================================================================ phase 1c: convex hard-overlap items
+    // ================================================================ phase 1c: convex hard-overlap items (a6)
     if (ANISO) {
       __syncthreads();
       const uint32_t nh = min(s_scal[3], (uint32_t)HCAP);
       for (uint32_t i = t; i < nh; i += T) {
-        const uint32_t it = s_hitems[i];
-        const uint32_t sl = it >> 16, pe = it & 0xffffu;
+        const uint32_t itm = s_hitems[i];
+        const uint32_t sl = itm >> 16, pe = itm & 0xffffu;
         const float4 r = s_pool[pe * E], ax = s_pool[pe * E + 1], an = s_anew[sl];
         if (mpr_overlap<SHAPE>(g, V3{r.x, r.y, r.z}, V3{an.x, an.y, an.z}, V3{ax.x, ax.y, ax.z}))
           s_state[sl] = OUT_HARD;
       }
-      __syncthreads();
-      for (int e = t; e < nlist; e += T)
-        if (s_state[e] == OUT_NONE && s_Nd[e] != 0) s_alive[atomicAdd(&s_scal[0], 1u)] = (uint16_t)e;
+    }
+    __syncthreads();
+    // ================================================================ phase 1d: N_d by table inversion (a7)
+#pragma unroll 1
+    for (int e = t; e < nlist; e += T) {
+      uint32_t Nd = 0;
+      if (s_state[e] == OUT_NONE && A.pt_n > 0) {
+        const uint32_t pid = __float_as_uint(s_r1[e].w);
+        const Block4 rn = philox(A.key, pid, 0, 0, P_NDEP + colw);
+        ++n_blocks;
+        const unsigned long long U = ((unsigned long long)rn.x << 32) | rn.y;
+        Nd = A.pt_klo + poisson_count(A.ptable, A.pt_n, Q.pguide, U);
+      }
+      s_Nd[e] = Nd; s_knext[e] = 0; s_rejmin[e] = 0xffffffffu;
+      if (s_state[e] == OUT_NONE && Nd != 0) s_alive[atomicAdd(&s_scal[0], 1u)] = (uint16_t)e;
     }
     __syncthreads();
     const int nalive = (int)s_scal[0];
