@@ -42,7 +42,8 @@ class Counters(C.Structure):
 
 
 def library_path() -> str:
-    return os.path.join(_HERE, "libhpmc_b200.so")
+    """In-tree library; HPMC_LIBRARY_PATH selects another build of the same sources (tuning builds)."""
+    return os.environ.get("HPMC_LIBRARY_PATH") or os.path.join(_HERE, "libhpmc_b200.so")
 
 
 def load_library() -> C.CDLL:

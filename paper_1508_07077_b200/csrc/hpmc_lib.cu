@@ -213,6 +213,7 @@ int launch_moveq(hpmc_ctx* ctx, const MoveArgs& a, const PoissonTable* pt) {
   if ((a.hc & (a.hc - 1)) == 0) q.magic_hc = (1ull << 63) / (unsigned long long)a.hc * 2ull + 1ull;
   q.pguide = pt->has_guide ? pt->d_G : nullptr;
   q.tile_cells = ctx->q_tile_cells;
+  q.wlo = 2.1f * a.g.w; q.whi = a.g.L - 2.1f * a.g.w;
   q.ntiles = (a.nact + q.tile_cells - 1) / q.tile_cells;
   {
     const float rl = (ctx->p.sigma_c + ctx->p.sigma_d) + 1e-3f;

@@ -42,6 +42,7 @@ struct QArgs {
   MoveArgs m;
   unsigned long long magic_hc;     // floor(2^64 / hc) + 1: exact a / hc by __umul64hi for a < 2^32
   const uint16_t* pguide;          // [1025] G[i] = #{j : T[j] < i 2^54}, or nullptr (plain binary search)
+  float wlo, whi;                  // 2.1 w and L - 2.1 w: centres in between need no minimum image (phase 1b)
   int tile_cells;                  // active cells per tile, <= T
   int ntiles;
   float rlist2;                    // neighbours farther than this from the new centre cannot touch any depletant
@@ -77,7 +78,7 @@ struct QSmem {
   static constexpr size_t o_aold = o_q1 + (Lq::ANISO ? sizeof(float4) * M : 0); // float4[M]
   static constexpr size_t o_anew = o_aold + (Lq::ANISO ? sizeof(float4) * M : 0);
   static constexpr size_t o_pool = o_anew + (Lq::ANISO ? sizeof(float4) * M : 0);
-  static constexpr size_t o_cell = o_pool + sizeof(float4) * (size_t)POOL * Lq::ENTRY;   // u32[M] ix|iy<<10|iz<<20|rot<<30
+  static constexpr size_t o_cell = o_pool + sizeof(float4) * (size_t)POOL * Lq::ENTRY;   // u32[M] ix|iy<<10|iz<<20|rot<<30|interior<<31
   static constexpr size_t o_Nd = o_cell + 4 * M;
   static constexpr size_t o_knext = o_Nd + 4 * M;
   static constexpr size_t o_rejmin = o_knext + 4 * M;
@@ -209,7 +210,12 @@ __global__ void __launch_bounds__(T) k_moveq(const QArgs Q) {
             s_r1[e] = make_float4(r1.x, r1.y, r1.z, p0.w);
             s_rho[e] = make_float4(minimg1(g, r0.x - r1.x), minimg1(g, r0.y - r1.y), minimg1(g, r0.z - r1.z),
                                    __uint_as_float(slot));
-            s_cell[e] = (uint32_t)ix | ((uint32_t)iy << 10) | ((uint32_t)iz << 20) | (rot ? (1u << 30) : 0u);
+            // interior: the new centre is more than two cell widths from the coordinate wrap on every axis, so the
+            // minimum image of any neighbour of the 27 cells is the plain difference (|d| < 2w <= L/3 < L/2; n_c >= 6)
+            const bool interior = nc >= 6 && r1.x > Q.wlo && r1.x < Q.whi && r1.y > Q.wlo && r1.y < Q.whi &&
+                                  r1.z > Q.wlo && r1.z < Q.whi;
+            s_cell[e] = (uint32_t)ix | ((uint32_t)iy << 10) | ((uint32_t)iz << 20) | (rot ? (1u << 30) : 0u) |
+                        (interior ? (1u << 31) : 0u);
             s_head[e] = -1;
             s_state[e] = OUT_NONE;
             if (ANISO) {
@@ -234,6 +240,7 @@ __global__ void __launch_bounds__(T) k_moveq(const QArgs Q) {
       const uint32_t slot = __float_as_uint(s_rho[e].w);
       const uint32_t cw = s_cell[e];
       const int ix = cw & 1023, iy = (cw >> 10) & 1023, iz = (cw >> 20) & 1023;
+      const bool interior = (cw >> 31) != 0u;
       const int dz = row / 3 - 1, dy = row - 3 * (row / 3) - 1;
       int jy = iy + dy, jz = iz + dz;
       jy += (jy < 0) ? nc : 0; jy -= (jy >= nc) ? nc : 0;
@@ -258,7 +265,8 @@ __global__ void __launch_bounds__(T) k_moveq(const QArgs Q) {
           for (int i = 0; i < 4; ++i) {
             const uint32_t s = s0 + i;
             if (s >= se || s == slot) continue;
-            const V3 rho = V3{minimg1(g, pj[i].x - r1.x), minimg1(g, pj[i].y - r1.y), minimg1(g, pj[i].z - r1.z)};
+            V3 rho = V3{pj[i].x - r1.x, pj[i].y - r1.y, pj[i].z - r1.z};
+            if (!interior) rho = V3{minimg1(g, rho.x), minimg1(g, rho.y), minimg1(g, rho.z)};
             const float r2 = dot3(rho, rho);
             if (!(r2 < Q.rlist2)) continue;
             if (!ANISO && r2 < g.dcirc2) { s_state[e] = OUT_HARD; continue; }     // a6 (spheres)
