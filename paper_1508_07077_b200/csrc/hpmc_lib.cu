@@ -31,7 +31,7 @@ struct PoissonTable {
   uint32_t k_lo = 0;
   int n = 0;
   unsigned long long* d_T = nullptr;
-  uint16_t* d_G = nullptr;              // guide table (1025 entries) or nullptr when the table has > 65535 entries
+  uint4* d_G = nullptr;                 // guide table (4096 buckets, see poisson_count in moveq.cuh)
   bool has_guide = false;
   size_t cap = 0;
 };
@@ -66,7 +66,7 @@ struct hpmc_ctx {
   int move_ctas = 0;
   unsigned int* d_tiles = nullptr;     // 8 tile counters, one per pass of a sweep
   int q_ctas = 0;                      // CTAs of the item-queue move kernel
-  int q_tile_cells = 0;                // active cells per tile (one wave)
+  int q_cpc = 0, q_big = 0, q_small = 0;   // active cells per CTA (one wave), tile sizes
   bool use_queue = true;               // HPMC_MOVE_KERNEL=warp selects the first (warp-per-cell) design
   int64_t launches = 0;
   bool timing = false;
@@ -157,18 +157,22 @@ int get_table(hpmc_ctx* ctx, double lambda, PoissonTable** out) {
   if (!T.empty()) {
     // pageable source: the runtime stages it before returning, so T may go out of scope
     CU(cudaMemcpyAsync(slot->d_T, T.data(), T.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice, ctx->stream));
-    if (T.size() <= 65535) {
-      // guide table: G[i] = #{j : T[j] < i 2^54}; the count for a uniform U with top bits b lies in [G[b], G[b+1]]
-      std::vector<uint16_t> G(1025);
+    {
+      // guide table: bucket b covers uniforms U with U >> 52 == b; {lo = #{j : T[j] < b 2^52}, n = thresholds inside
+      // the bucket, T[lo] low word, T[lo] high word}
+      std::vector<uint4> G(4096);
       size_t j = 0;
-      for (unsigned i = 0; i < 1024; ++i) {
-        const unsigned long long edge = (unsigned long long)i << 54;
+      for (unsigned i = 0; i < 4096; ++i) {
+        const unsigned long long edge = (unsigned long long)i << 52;
         while (j < T.size() && T[j] < edge) ++j;
-        G[i] = (uint16_t)j;
+        size_t j2 = j;
+        if (i == 4095) j2 = T.size();
+        else { const unsigned long long e2 = (unsigned long long)(i + 1) << 52; while (j2 < T.size() && T[j2] < e2) ++j2; }
+        const unsigned long long t0 = j < T.size() ? T[j] : ~0ull;
+        G[i] = make_uint4((unsigned)j, (unsigned)(j2 - j), (unsigned)(t0 & 0xffffffffull), (unsigned)(t0 >> 32));
       }
-      G[1024] = (uint16_t)T.size();
-      if (!slot->d_G) CU(cudaMalloc(&slot->d_G, 1025 * sizeof(uint16_t)));
-      CU(cudaMemcpyAsync(slot->d_G, G.data(), 1025 * sizeof(uint16_t), cudaMemcpyHostToDevice, ctx->stream));
+      if (!slot->d_G) CU(cudaMalloc(&slot->d_G, 4096 * sizeof(uint4)));
+      CU(cudaMemcpyAsync(slot->d_G, G.data(), 4096 * sizeof(uint4), cudaMemcpyHostToDevice, ctx->stream));
       slot->has_guide = true;
     }
     CU(cudaStreamSynchronize(ctx->stream));
@@ -188,20 +192,24 @@ int setup_moveq(hpmc_ctx* ctx) {
   int per_sm = 0;
   e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_moveq<SHAPE, QT>, QT, smem);
   if (e != cudaSuccess || per_sm < 1) return fail(ctx, HPMC_E_CUDA, "k_moveq does not fit on an SM");
-  // one wave: tiles sized so that every tile of a pass is resident at once (a pass is latency-, not throughput-bound)
+  // one wave: every CTA of a pass is resident at once (a pass is latency-, not throughput-bound) and owns
+  // cells_per_cta active cells, worked through in nsub tiles of equal size
   const int nact = ctx->ncell / 8;
   const int resident = ctx->num_sms * per_sm;
-  const long long waves = ((long long)nact + (long long)resident * QT - 1) / ((long long)resident * QT);
-  int tc = (int)((nact + waves * resident - 1) / (waves * resident));   // every CTA gets `waves` tiles of equal size
-  if (tc < 16) tc = 16;
-  if (tc > QT) tc = QT;
-  if (const char* o = getenv("HPMC_TILE_CELLS")) { const int v = atoi(o); if (v >= 1 && v <= QT) tc = v; }
-  ctx->q_tile_cells = tc;
-  const int ntiles = (nact + tc - 1) / tc;
-  ctx->q_ctas = ntiles < resident ? ntiles : resident;
+  int cpc = (nact + resident - 1) / resident;
+  if (cpc < 32) cpc = 32;
+  int nsub = (cpc + QT - 1) / QT;
+  if (nsub < 2 && cpc > 48) nsub = 2;
+  int big = (cpc + nsub - 1) / nsub;
+  if (big > QT) big = QT;
+  int small = big;
+  if (const char* o = getenv("HPMC_TILE_BIG")) { const int v = atoi(o); if (v >= 1 && v <= QT) big = v; }
+  if (const char* o = getenv("HPMC_TILE_SMALL")) { const int v = atoi(o); if (v >= 1 && v <= QT) small = v; }
+  ctx->q_cpc = cpc; ctx->q_big = big; ctx->q_small = small;
+  ctx->q_ctas = (nact + cpc - 1) / cpc;
   if (getenv("HPMC_VERBOSE"))
-    fprintf(stderr, "k_moveq<%d,%d>: smem %zu B, %d CTAs/SM, tile %d cells, %d tiles, %d CTAs\n", SHAPE, QT, smem, per_sm, tc,
-            ntiles, ctx->q_ctas);
+    fprintf(stderr, "k_moveq<%d,%d>: smem %zu B, %d CTAs/SM, %d CTAs x %d cells, tiles %d (odd CTAs start with %d)\n", SHAPE,
+            QT, smem, per_sm, ctx->q_ctas, cpc, big, small);
   return 0;
 }
 
@@ -212,9 +220,8 @@ int launch_moveq(hpmc_ctx* ctx, const MoveArgs& a, const PoissonTable* pt) {
   q.magic_hc = ~0ull / (unsigned long long)a.hc + 1ull;   // floor((2^64-1)/hc)+1 == floor(2^64/hc)+1 unless hc | 2^64
   if ((a.hc & (a.hc - 1)) == 0) q.magic_hc = (1ull << 63) / (unsigned long long)a.hc * 2ull + 1ull;
   q.pguide = pt->has_guide ? pt->d_G : nullptr;
-  q.tile_cells = ctx->q_tile_cells;
+  q.cells_per_cta = ctx->q_cpc; q.tile_big = ctx->q_big; q.tile_small = ctx->q_small;
   q.wlo = 2.1f * a.g.w; q.whi = a.g.L - 2.1f * a.g.w;
-  q.ntiles = (a.nact + q.tile_cells - 1) / q.tile_cells;
   {
     const float rl = (ctx->p.sigma_c + ctx->p.sigma_d) + 1e-3f;
     q.rlist2 = rl * rl;

@@ -3,8 +3,8 @@
 // C3 has 175,616 active cells per pass and a B200 holds ~300k resident threads, so a pass is ONE wave of work: its
 // duration is the serial latency chain of a tile, not a throughput.  The kernel is therefore organised to keep every
 // chain short and every phase spread over all T lanes of the CTA:
-//   tiling   tiles of `tile_cells` <= T active cells, sized by the host so that all tiles are resident at once
-//            (one wave, static assignment tile = blockIdx.x + i gridDim.x: no tile counter, no second-tile tail).
+//   tiling   every CTA owns a contiguous range of active cells, sized by the host so that all CTAs are resident at
+//            once (one wave, no tile counter), and works through it in tiles of <= T cells.
 //   phase 1a one THREAD per active cell: pick (a3), trial pose + confinement (a4).  Moves that stay in their cell are
 //            compacted into a dense list in shared memory (empty cells and boundary rejections drop out here).
 //   phase 1b one thread per (move, x-row) item, 9 rows per move: the row's 3 cells are one contiguous span of the
@@ -41,10 +41,12 @@ namespace hpmc {
 struct QArgs {
   MoveArgs m;
   unsigned long long magic_hc;     // floor(2^64 / hc) + 1: exact a / hc by __umul64hi for a < 2^32
-  const uint16_t* pguide;          // [1025] G[i] = #{j : T[j] < i 2^54}, or nullptr (plain binary search)
+  const uint4* pguide;             // [4096] guide table of the Poisson thresholds (poisson_count), or nullptr
   float wlo, whi;                  // 2.1 w and L - 2.1 w: centres in between need no minimum image (phase 1b)
-  int tile_cells;                  // active cells per tile, <= T
-  int ntiles;
+  int cells_per_cta;               // CTA b owns the active cells [b cells_per_cta, (b+1) cells_per_cta)
+  int tile_big, tile_small;        // ... and works through them in tiles of tile_big <= T cells; odd CTAs start with
+                                   // one tile of tile_small cells (a phase stagger between neighbouring CTAs; measured
+                                   // neutral at C3, so the host sets tile_small = tile_big)
   float rlist2;                    // neighbours farther than this from the new centre cannot touch any depletant
                                    // of the move: (sigma_c + sigma_d + 1e-3)^2 for the plain rule (insertion
                                    // sphere about the new centre only), r_cut^2 of R-3.4 otherwise
@@ -109,13 +111,18 @@ __device__ __forceinline__ bool q_free_of_nbrs(const Geo& g, const float4* pool,
   return true;
 }
 
-// N_d = k_lo + #{j : T[j] <= U} (R-S2).  With the guide table the search starts from the bucket of U's top 10 bits.
+// N_d = k_lo + #{j : T[j] <= U} (R-S2).  Guide table: bucket b = U >> 52 holds {lo = #{T < b 2^52}, n = number of
+// thresholds inside the bucket, T[lo] as two words}: one 16-byte load answers the common case (n <= 1); a bucket with
+// more thresholds (the far tails of the distribution) falls back to a binary search over its n entries.
 __device__ __forceinline__ uint32_t poisson_count(const unsigned long long* __restrict__ T, int n,
-                                                  const uint16_t* __restrict__ guide, unsigned long long U) {
+                                                  const uint4* __restrict__ guide, unsigned long long U) {
   int lo = 0, hi = n;
   if (guide) {
-    const uint32_t b = (uint32_t)(U >> 54);
-    lo = __ldg(&guide[b]); hi = __ldg(&guide[b + 1]);
+    const uint4 gb = __ldg(&guide[(uint32_t)(U >> 52)]);
+    const unsigned long long t0 = ((unsigned long long)gb.w << 32) | gb.z;
+    if (gb.y == 0u || U < t0) return gb.x;
+    if (gb.y == 1u) return gb.x + 1u;
+    lo = (int)gb.x + 1; hi = (int)(gb.x + gb.y);
   }
   while (lo < hi) {
     const int mid = (lo + hi) >> 1;
@@ -163,14 +170,20 @@ __global__ void __launch_bounds__(T) k_moveq(const QArgs Q) {
   uint32_t n_tt = 0, n_at = 0, n_tr = 0, n_ar = 0, n_rb = 0, n_rh = 0, n_rd = 0;
   uint32_t n_drawn = 0, n_needed = 0, n_eval = 0, n_blocks = 0;
 
-  for (uint32_t tile = blockIdx.x; tile < (uint32_t)Q.ntiles; tile += gridDim.x) {
+  const uint32_t cta_lo = blockIdx.x * (uint32_t)Q.cells_per_cta;
+  const uint32_t cta_hi = min(cta_lo + (uint32_t)Q.cells_per_cta, (uint32_t)A.nact);
+  bool first_tile = true;
+  for (uint32_t cur = cta_lo; cur < cta_hi;) {
+    const uint32_t tile_n = min((first_tile && (blockIdx.x & 1u)) ? (uint32_t)Q.tile_small : (uint32_t)Q.tile_big, cta_hi - cur);
+    const uint32_t tile_lo = cur;
+    cur += tile_n; first_tile = false;
     if (t == 0) { s_scal[0] = 0; s_scal[1] = 0; s_scal[3] = 0; s_scal[4] = 0; }
     __syncthreads();
 
     // ================================================================ phase 1a: one thread per active cell
-    if (t < Q.tile_cells) {
-      const uint32_t a = tile * (uint32_t)Q.tile_cells + (uint32_t)t;
-      if (a < (uint32_t)A.nact) {
+    if ((uint32_t)t < tile_n) {
+      const uint32_t a = tile_lo + (uint32_t)t;
+      {
         const uint32_t q1d = (uint32_t)__umul64hi((unsigned long long)a, Q.magic_hc);        // a / hc
         const uint32_t q2d = (uint32_t)__umul64hi((unsigned long long)q1d, Q.magic_hc);      // a / hc^2
         const int ix = 2 * (int)(a - q1d * hc) + px, iy = 2 * (int)(q1d - q2d * hc) + py, iz = 2 * (int)q2d + pz;
