@@ -1,8 +1,7 @@
 // moveq.cuh -- steps a3..a10, item-queue design of the checkerboard move kernel (K-B).
 //
-// C3 has 175,616 active cells per pass and a B200 holds ~300k resident threads, so a pass is ONE wave of work: its
-// duration is the serial latency chain of a tile, not a throughput.  The kernel is therefore organised to keep every
-// chain short and every phase spread over all T lanes of the CTA:
+// C3 has 175,616 active cells per pass and a B200 holds ~150k resident threads of this kernel, so a pass is ONE wave
+// of work.  Every phase is spread over all T lanes of the CTA and every dependent-load chain is kept short:
 //   tiling   every CTA owns a contiguous range of active cells, sized by the host so that all CTAs are resident at
 //            once (one wave, no tile counter), and works through it in tiles of <= T cells.
 //   phase 1a one THREAD per active cell: pick (a3), trial pose + confinement (a4).  Moves that stay in their cell are
@@ -13,8 +12,8 @@
 //            the move's linked list in a CTA-wide shared-memory pool.
 //   phase 1c (convex shapes) the (move, neighbour) pairs inside the circumsphere distance are items of their own;
 //            the CTA's lanes run the support-function test on them side by side.
-//   phase 1d one thread per move: N_d by table inversion (a7), three dependent loads instead of eleven thanks to a
-//            1024-bucket guide table indexed by the top 10 bits of the uniform.
+//   phase 1d one thread per move: N_d by table inversion (a7), one 16-byte load instead of an eleven-step binary
+//            search thanks to a 4096-bucket guide table indexed by the top 12 bits of the uniform.
 //   phase 2  the depletant insertions of ALL surviving moves of the tile are one pool of items
 //            (move m, depletant k, attempt a).  Every lane repeatedly claims the next k of the move it is
 //            attached to (shared-memory atomic), computes ONE Philox block per loop trip, and on an accepted
