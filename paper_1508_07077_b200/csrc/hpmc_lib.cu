@@ -182,15 +182,19 @@ int get_table(hpmc_ctx* ctx, double lambda, PoissonTable** out) {
   return 0;
 }
 
+#ifndef HPMC_QCPT
+#define HPMC_QCPT 2
+#endif
 constexpr int QT = 128;                // threads per CTA of the item-queue kernel
+template <int SHAPE> struct QCfg { static constexpr int CPT = SHAPE == SH_SPHERE ? HPMC_QCPT : 1; };   // tile capacity CPT*QT cells
 
 template <int SHAPE>
 int setup_moveq(hpmc_ctx* ctx) {
-  const size_t smem = QSmem<SHAPE, QT>::bytes;
-  cudaError_t e = cudaFuncSetAttribute(k_moveq<SHAPE, QT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  const size_t smem = QSmem<SHAPE, QT, QCfg<SHAPE>::CPT>::bytes;
+  cudaError_t e = cudaFuncSetAttribute(k_moveq<SHAPE, QT, QCfg<SHAPE>::CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return fail(ctx, HPMC_E_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
   int per_sm = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_moveq<SHAPE, QT>, QT, smem);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_moveq<SHAPE, QT, QCfg<SHAPE>::CPT>, QT, smem);
   if (e != cudaSuccess || per_sm < 1) return fail(ctx, HPMC_E_CUDA, "k_moveq does not fit on an SM");
   // one wave: every CTA of a pass is resident at once (a pass is latency-, not throughput-bound) and owns
   // cells_per_cta active cells, worked through in nsub tiles of equal size
@@ -198,13 +202,13 @@ int setup_moveq(hpmc_ctx* ctx) {
   const int resident = ctx->num_sms * per_sm;
   int cpc = (nact + resident - 1) / resident;
   if (cpc < 32) cpc = 32;
-  int nsub = (cpc + QT - 1) / QT;
-  if (nsub < 2 && cpc > 48) nsub = 2;
+  constexpr int QM = QCfg<SHAPE>::CPT * QT;
+  int nsub = (cpc + QM - 1) / QM;
   int big = (cpc + nsub - 1) / nsub;
-  if (big > QT) big = QT;
+  if (big > QM) big = QM;
   int small = big;
-  if (const char* o = getenv("HPMC_TILE_BIG")) { const int v = atoi(o); if (v >= 1 && v <= QT) big = v; }
-  if (const char* o = getenv("HPMC_TILE_SMALL")) { const int v = atoi(o); if (v >= 1 && v <= QT) small = v; }
+  if (const char* o = getenv("HPMC_TILE_BIG")) { const int v = atoi(o); if (v >= 1 && v <= QM) big = v; }
+  if (const char* o = getenv("HPMC_TILE_SMALL")) { const int v = atoi(o); if (v >= 1 && v <= QM) small = v; }
   ctx->q_cpc = cpc; ctx->q_big = big; ctx->q_small = small;
   ctx->q_ctas = (nact + cpc - 1) / cpc;
   if (getenv("HPMC_VERBOSE"))
@@ -227,7 +231,7 @@ int launch_moveq(hpmc_ctx* ctx, const MoveArgs& a, const PoissonTable* pt) {
     q.rlist2 = rl * rl;
     if (q.rlist2 > a.g.rcut2) q.rlist2 = a.g.rcut2;
   }
-  k_moveq<SHAPE, QT><<<ctx->q_ctas, QT, QSmem<SHAPE, QT>::bytes, ctx->stream>>>(q);
+  k_moveq<SHAPE, QT, QCfg<SHAPE>::CPT><<<ctx->q_ctas, QT, QSmem<SHAPE, QT, QCfg<SHAPE>::CPT>::bytes, ctx->stream>>>(q);
   return 0;
 }
 

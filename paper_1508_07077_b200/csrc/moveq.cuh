@@ -43,7 +43,7 @@ struct QArgs {
   const uint4* pguide;             // [4096] guide table of the Poisson thresholds (poisson_count), or nullptr
   float wlo, whi;                  // 2.1 w and L - 2.1 w: centres in between need no minimum image (phase 1b)
   int cells_per_cta;               // CTA b owns the active cells [b cells_per_cta, (b+1) cells_per_cta)
-  int tile_big, tile_small;        // ... and works through them in tiles of tile_big <= T cells; odd CTAs start with
+  int tile_big, tile_small;        // ... and works through them in tiles of tile_big <= CPT*T cells; odd CTAs start with
                                    // one tile of tile_small cells (a phase stagger between neighbouring CTAs; measured
                                    // neutral at C3, so the host sets tile_small = tile_big)
   float rlist2;                    // neighbours farther than this from the new centre cannot touch any depletant
@@ -58,19 +58,24 @@ __device__ __forceinline__ float sym_unit_bits(uint32_t x) {
   return fmaf(f - 1.5f, 2.0f, 1.1920928955078125e-07f);
 }
 
+#ifndef HPMC_WALK_SLOTS
+#define HPMC_WALK_SLOTS 4         // phase 1b: particle loads in flight per (move, row) item
+#endif
+
 template <int SHAPE>
 struct QLayout {
   static constexpr bool ANISO = SHAPE != SH_SPHERE;
   static constexpr int ENTRY = ANISO ? 2 : 1;                 // float4 per neighbour entry
   static constexpr int POOL_PER_MOVE = ANISO ? 12 : 6;        // pool capacity = this x T entries (tile average)
   static constexpr int HCAP_PER_MOVE = 4;                     // hard-test items (convex shapes) = this x T
+  static constexpr int MIN_CTAS = ANISO ? 1 : 8;              // resident CTAs per SM the register allocation must allow
 };
 
-// shared-memory carve-up for a CTA of T threads handling up to M = T moves per tile
-template <int SHAPE, int T>
+// shared-memory carve-up for a CTA of T threads handling tiles of up to M = CPT*T active cells (hence <= M moves)
+template <int SHAPE, int T, int CPT>
 struct QSmem {
   using Lq = QLayout<SHAPE>;
-  static constexpr int M = T;
+  static constexpr int M = CPT * T;
   static constexpr int POOL = Lq::POOL_PER_MOVE * T;
   static constexpr int HCAP = Lq::ANISO ? Lq::HCAP_PER_MOVE * T : 0;
   static constexpr size_t o_r1 = 0;                                             // float4[M]  r1.xyz, pid bits
@@ -130,13 +135,14 @@ __device__ __forceinline__ uint32_t poisson_count(const unsigned long long* __re
   return (uint32_t)lo;
 }
 
-template <int SHAPE, int T>
-__global__ void __launch_bounds__(T) k_moveq(const QArgs Q) {
+template <int SHAPE, int T, int CPT>
+__global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QArgs Q) {
   using Lq = QLayout<SHAPE>;
-  using S = QSmem<SHAPE, T>;
+  using S = QSmem<SHAPE, T, CPT>;
   constexpr bool ANISO = Lq::ANISO;
   constexpr int E = Lq::ENTRY;
   constexpr int M = S::M, POOL = S::POOL, HCAP = S::HCAP, NW = M / 32;
+  constexpr int SLOTS = HPMC_WALK_SLOTS;
   const MoveArgs& A = Q.m;
   const Geo& g = A.g;
 
@@ -180,8 +186,9 @@ __global__ void __launch_bounds__(T) k_moveq(const QArgs Q) {
     __syncthreads();
 
     // ================================================================ phase 1a: one thread per active cell
-    if ((uint32_t)t < tile_n) {
-      const uint32_t a = tile_lo + (uint32_t)t;
+#pragma unroll 1
+    for (uint32_t c = t; c < tile_n; c += T) {
+      const uint32_t a = tile_lo + c;
       {
         const uint32_t q1d = (uint32_t)__umul64hi((unsigned long long)a, Q.magic_hc);        // a / hc
         const uint32_t q2d = (uint32_t)__umul64hi((unsigned long long)q1d, Q.magic_hc);      // a / hc^2
@@ -262,40 +269,44 @@ __global__ void __launch_bounds__(T) k_moveq(const QArgs Q) {
       int x0 = ix - 1, n0 = 3, n1 = 0;
       if (ix == 0) { x0 = nc - 1; n0 = 1; n1 = 2; }
       else if (ix == nc - 1) { x0 = nc - 2; n0 = 2; n1 = 1; }
+      // one virtual span: the main part [sb0, sb0+len0) followed by the wrapped part [sb1, sb1+len1) (rare)
+      const uint32_t sb0 = A.cell_start[rb + x0], len0 = A.cell_start[rb + x0 + n0] - sb0;
+      uint32_t sb1 = 0, len1 = 0;
+      if (n1 != 0) { sb1 = A.cell_start[rb]; len1 = A.cell_start[rb + n1] - sb1; }
+      const uint32_t len = len0 + len1;
+      // SLOTS particles in flight per trip (a row holds 2.2 particles on average at C3; more slots cost registers and
+      // with them a resident CTA per SM: 4 and 5 measured equal, 6 and 8 slower)
 #pragma unroll 1
-      for (int seg = 0; seg < 2; ++seg) {
-        const int xs = seg ? 0 : x0, nn = seg ? n1 : n0;
-        if (nn == 0) break;
-        const uint32_t sb = A.cell_start[rb + xs], se = A.cell_start[rb + xs + nn];
-#pragma unroll 1
-        for (uint32_t s0 = sb; s0 < se; s0 += 4) {
-          float4 pj[4];
+      for (uint32_t i0 = 0; i0 < len; i0 += SLOTS) {
+        float4 pj[SLOTS];
 #pragma unroll
-          for (int i = 0; i < 4; ++i)
-            if (s0 + i < se) pj[i] = A.cpos[s0 + i];
+        for (int u = 0; u < SLOTS; ++u) {
+          const uint32_t i = i0 + u;
+          if (i < len) pj[u] = A.cpos[i < len0 ? sb0 + i : sb1 + (i - len0)];
+        }
 #pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const uint32_t s = s0 + i;
-            if (s >= se || s == slot) continue;
-            V3 rho = V3{pj[i].x - r1.x, pj[i].y - r1.y, pj[i].z - r1.z};
-            if (!interior) rho = V3{minimg1(g, rho.x), minimg1(g, rho.y), minimg1(g, rho.z)};
-            const float r2 = dot3(rho, rho);
-            if (!(r2 < Q.rlist2)) continue;
-            if (!ANISO && r2 < g.dcirc2) { s_state[e] = OUT_HARD; continue; }     // a6 (spheres)
-            const int pe = (int)atomicAdd(&s_scal[1], 1u);
-            if (pe >= POOL) { atomicExch(A.err_flag, 1); continue; }
-            const int prev = atomicExch(&s_head[e], pe);
-            s_pool[pe * E] = make_float4(rho.x, rho.y, rho.z, __int_as_float(prev));
-            if (ANISO) {
-              const float4 axj = A.caxis[s];
-              s_pool[pe * E + 1] = axj;
-              if (r2 < g.dcirc2) {
-                const uint32_t hi = atomicAdd(&s_scal[3], 1u);
-                if (hi < (uint32_t)HCAP) s_hitems[hi] = ((uint32_t)e << 16) | (uint32_t)pe;
-                else {
-                  const float4 an = s_anew[e];
-                  if (mpr_overlap<SHAPE>(g, rho, V3{an.x, an.y, an.z}, V3{axj.x, axj.y, axj.z})) s_state[e] = OUT_HARD;
-                }
+        for (int u = 0; u < SLOTS; ++u) {
+          const uint32_t i = i0 + u;
+          const uint32_t s = i < len0 ? sb0 + i : sb1 + (i - len0);
+          if (i >= len || s == slot) continue;
+          V3 rho = V3{pj[u].x - r1.x, pj[u].y - r1.y, pj[u].z - r1.z};
+          if (!interior) rho = V3{minimg1(g, rho.x), minimg1(g, rho.y), minimg1(g, rho.z)};
+          const float r2 = dot3(rho, rho);
+          if (!(r2 < Q.rlist2)) continue;
+          if (!ANISO && r2 < g.dcirc2) { s_state[e] = OUT_HARD; continue; }     // a6 (spheres)
+          const int pe = (int)atomicAdd(&s_scal[1], 1u);
+          if (pe >= POOL) { atomicExch(A.err_flag, 1); continue; }
+          const int prev = atomicExch(&s_head[e], pe);
+          s_pool[pe * E] = make_float4(rho.x, rho.y, rho.z, __int_as_float(prev));
+          if (ANISO) {
+            const float4 axj = A.caxis[s];
+            s_pool[pe * E + 1] = axj;
+            if (r2 < g.dcirc2) {
+              const uint32_t hi = atomicAdd(&s_scal[3], 1u);
+              if (hi < (uint32_t)HCAP) s_hitems[hi] = ((uint32_t)e << 16) | (uint32_t)pe;
+              else {
+                const float4 an = s_anew[e];
+                if (mpr_overlap<SHAPE>(g, rho, V3{an.x, an.y, an.z}, V3{axj.x, axj.y, axj.z})) s_state[e] = OUT_HARD;
               }
             }
           }
