@@ -138,9 +138,10 @@ int hpmc_step_host(hpmc_ctx* ctx, float* host_pos4, float* host_quat4, uint8_t* 
 /* Number of kernel launches the library has enqueued since init (for bench.py's gpu_launches). */
 int64_t hpmc_launch_count(hpmc_ctx* ctx);
 
-/* Event timing of the move kernel (the dominant kernel): while enabled, every move-kernel launch is bracketed
- * by CUDA events on the context's stream; hpmc_move_kernel_ms synchronises and returns the accumulated
- * milliseconds and launch count since enabling. */
+/* Event timing of the move kernel (the dominant kernel): while enabled, the 8 move-kernel launches of every sweep
+ * are bracketed by ONE pair of CUDA events on the context's stream (the gaps between the 8 launches are inside the
+ * bracket); hpmc_move_kernel_ms synchronises and returns the accumulated milliseconds and the number of launches
+ * (8 per sweep) since enabling. */
 int hpmc_time_move_kernel(hpmc_ctx* ctx, int32_t enable);
 int hpmc_move_kernel_ms(hpmc_ctx* ctx, double* ms_total, int64_t* launches);
 

@@ -202,6 +202,7 @@ int setup_moveq(hpmc_ctx* ctx) {
   const int resident = ctx->num_sms * per_sm;
   int cpc = (nact + resident - 1) / resident;
   if (cpc < 32) cpc = 32;
+  if (const char* o = getenv("HPMC_CELLS_PER_CTA")) { const int v = atoi(o); if (v >= 1) cpc = v; }
   constexpr int QM = QCfg<SHAPE>::CPT * QT;
   int nsub = (cpc + QM - 1) / QM;
   int big = (cpc + nsub - 1) / nsub;
@@ -397,18 +398,20 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
   a.ptable = pt->d_T; a.pt_n = pt->n; a.pt_klo = pt->k_lo;
   a.outcome = ctx->d_outcome; a.counters = ctx->d_counters; a.err_flag = ctx->d_err;
   const bool cb = n_trial > 0;
+  // timing: ONE event pair around the 8 launches of the sweep (an event pair per launch costs more than the gaps
+  // between the launches it would exclude); hpmc_move_kernel_ms counts 8 launches per pair
+  EventPair* ep = nullptr;
+  if (ctx->timing) {
+    if (ctx->ev_used == ctx->ev.size()) {
+      EventPair e;
+      CU(cudaEventCreate(&e.a)); CU(cudaEventCreate(&e.b));
+      ctx->ev.push_back(e);
+    }
+    ep = &ctx->ev[ctx->ev_used++];
+    CU(cudaEventRecord(ep->a, ctx->stream));
+  }
   for (int pass = 0; pass < 8; ++pass) {
     a.colour = perm[pass];
-    EventPair* ep = nullptr;
-    if (ctx->timing) {
-      if (ctx->ev_used == ctx->ev.size()) {
-        EventPair e;
-        CU(cudaEventCreate(&e.a)); CU(cudaEventCreate(&e.b));
-        ctx->ev.push_back(e);
-      }
-      ep = &ctx->ev[ctx->ev_used++];
-      CU(cudaEventRecord(ep->a, ctx->stream));
-    }
     if (ctx->use_queue && !cb) {
       switch (ctx->p.shape) {
         case HPMC_SPHERE: launch_moveq<SH_SPHERE>(ctx, a, pt); break;
@@ -422,8 +425,8 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
         default: launch_move<SH_SPHERODISK>(ctx, a, cb); break;
       }
     }
-    if (ep) CU(cudaEventRecord(ep->b, ctx->stream));
   }
+  if (ep) CU(cudaEventRecord(ep->b, ctx->stream));
   ctx->launches += 8;
   CU(cudaGetLastError());
   ctx->built = false;
@@ -534,7 +537,7 @@ int hpmc_move_kernel_ms(hpmc_ctx* ctx, double* ms_total, int64_t* launches) {
     CU(cudaEventElapsedTime(&ms, ctx->ev[i].a, ctx->ev[i].b));
     ctx->ev_ms += ms;
   }
-  ctx->ev_launches += (int64_t)ctx->ev_used;
+  ctx->ev_launches += 8 * (int64_t)ctx->ev_used;
   ctx->ev_used = 0;
   *ms_total = ctx->ev_ms; *launches = ctx->ev_launches;
   return HPMC_OK;
