@@ -114,7 +114,8 @@ int hpmc_run(hpmc_ctx* ctx, uint32_t seed, uint32_t step0, int64_t n_sweeps, dou
 int hpmc_counters(hpmc_ctx* ctx, hpmc_counters_t* host_out);
 int hpmc_reset_counters(hpmc_ctx* ctx);
 
-/* Copy the outcome codes of the last sweep into d_outcome (device, N bytes, caller-owned).  Asynchronous. */
+/* Copy the outcome codes of the last sweep into d_outcome (device, N bytes, caller-owned).  Asynchronous.
+ * hpmc_build_cells resets the codes to HPMC_OUT_NONE for the sweep it prepares. */
 int hpmc_outcomes(hpmc_ctx* ctx, uint8_t* d_outcome);
 
 /* Grid geometry chosen at init: cells per axis and cell width. */

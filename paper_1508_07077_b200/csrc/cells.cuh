@@ -14,9 +14,10 @@ namespace hpmc {
 
 __global__ void __launch_bounds__(256) k_bin_count(const float4* __restrict__ pos, int N, Geo g, float sx, float sy,
                                                    float sz, uint32_t* __restrict__ cid, uint32_t* __restrict__ rank,
-                                                   uint32_t* __restrict__ counts) {
+                                                   uint32_t* __restrict__ counts, uint8_t* __restrict__ outcome) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= N) return;
+  outcome[i] = 0;                      // outcome codes of the sweep this build belongs to: "not tried"
   const float4 p = pos[i];
   const int ix = cell_axis(g, p.x, sx), iy = cell_axis(g, p.y, sy), iz = cell_axis(g, p.z, sz);
   const uint32_t c = ((uint32_t)iz * g.nc + iy) * g.nc + ix;
@@ -79,16 +80,37 @@ __global__ void __launch_bounds__(1024) k_scan_top(uint32_t* __restrict__ tile_s
   }
 }
 
-__global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(const uint32_t* __restrict__ counts, int n,
+// FUSED_TOP: tile_sums holds the raw tile totals and every CTA adds up the totals of the tiles before it (a few
+// hundred words from L2: cheaper than a launch of k_scan_top); otherwise tile_sums is already the exclusive scan.
+// The counts are consumed here for the last time and re-zeroed for the next build.
+template <bool FUSED_TOP>
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_apply(uint32_t* __restrict__ counts, int n,
                                                              const uint32_t* __restrict__ tile_sums,
                                                              uint32_t* __restrict__ cell_start) {
   __shared__ uint32_t s_warp[32];
+  __shared__ uint32_t s_off;
+  uint32_t off;
+  if (FUSED_TOP) {
+    uint32_t part = 0;
+    for (int i = threadIdx.x; i < (int)blockIdx.x; i += SCAN_THREADS) part += tile_sums[i];
+    uint32_t tot;
+    block_exclusive_scan(part, s_warp, tot);
+    if (threadIdx.x == 0) s_off = tot;
+    __syncthreads();
+    off = s_off;
+  } else {
+    off = tile_sums[blockIdx.x];
+  }
   const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
   uint32_t v[SCAN_ITEMS], s = 0;
 #pragma unroll
-  for (int k = 0; k < SCAN_ITEMS; ++k) { v[k] = (base + k < n) ? counts[base + k] : 0u; s += v[k]; }
+  for (int k = 0; k < SCAN_ITEMS; ++k) {
+    v[k] = (base + k < n) ? counts[base + k] : 0u;
+    s += v[k];
+    if (base + k < n) counts[base + k] = 0u;
+  }
   uint32_t total;
-  uint32_t run = tile_sums[blockIdx.x] + block_exclusive_scan(s, s_warp, total);
+  uint32_t run = off + block_exclusive_scan(s, s_warp, total);
 #pragma unroll
   for (int k = 0; k < SCAN_ITEMS; ++k) {
     if (base + k < n) cell_start[base + k] = run;

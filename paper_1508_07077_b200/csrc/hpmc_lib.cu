@@ -297,6 +297,7 @@ int hpmc_init(hpmc_ctx** out, const hpmc_params* p, int64_t N, float* d_pos4, fl
   CUI(cudaMalloc(&ctx->d_err, sizeof(int)));
   CUI(cudaMalloc(&ctx->d_tiles, sizeof(unsigned int) * 8));
   CUI(cudaMemsetAsync(ctx->d_outcome, 0, (size_t)N, ctx->stream));
+  CUI(cudaMemsetAsync(ctx->d_counts, 0, sizeof(uint32_t) * ctx->ncell, ctx->stream));   // kept zero between builds by k_scan_apply
   CUI(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * C_COUNT, ctx->stream));
   CUI(cudaMemsetAsync(ctx->d_err, 0, sizeof(int), ctx->stream));
 #undef CUI
@@ -343,12 +344,18 @@ int hpmc_build_cells(hpmc_ctx* ctx, uint32_t seed, uint32_t step) {
   ctx->shift[2] = unit01(r.z) * ctx->g.w;
   const int N = (int)ctx->N, nb = (N + 255) / 256;
   cudaStream_t st = ctx->stream;
-  CU(cudaMemsetAsync(ctx->d_counts, 0, sizeof(uint32_t) * ctx->ncell, st));
+  // d_counts is zero here: hpmc_init clears it once and k_scan_apply re-zeroes it after its last read
   k_bin_count<<<nb, 256, 0, st>>>(ctx->d_pos, N, ctx->g, ctx->shift[0], ctx->shift[1], ctx->shift[2], ctx->d_cid,
-                                  ctx->d_rank, ctx->d_counts);
+                                  ctx->d_rank, ctx->d_counts, ctx->d_outcome);
   k_scan_tiles<<<ctx->ntiles, SCAN_THREADS, 0, st>>>(ctx->d_counts, ctx->ncell, ctx->d_tile_sums);
-  k_scan_top<<<1, 1024, 0, st>>>(ctx->d_tile_sums, ctx->ntiles);
-  k_scan_apply<<<ctx->ntiles, SCAN_THREADS, 0, st>>>(ctx->d_counts, ctx->ncell, ctx->d_tile_sums, ctx->d_cell_start);
+  if (ctx->ntiles <= 4096) {
+    k_scan_apply<true><<<ctx->ntiles, SCAN_THREADS, 0, st>>>(ctx->d_counts, ctx->ncell, ctx->d_tile_sums, ctx->d_cell_start);
+    ctx->launches += 5;
+  } else {
+    k_scan_top<<<1, 1024, 0, st>>>(ctx->d_tile_sums, ctx->ntiles);
+    k_scan_apply<false><<<ctx->ntiles, SCAN_THREADS, 0, st>>>(ctx->d_counts, ctx->ncell, ctx->d_tile_sums, ctx->d_cell_start);
+    ctx->launches += 6;
+  }
   k_fill<<<nb, 256, 0, st>>>(ctx->d_cid, ctx->d_rank, ctx->d_cell_start, N, ctx->d_cell_pid);
   const int cbk = (ctx->ncell + 255) / 256;
   if (ctx->p.shape == HPMC_SPHERE)
@@ -357,7 +364,6 @@ int hpmc_build_cells(hpmc_ctx* ctx, uint32_t seed, uint32_t step) {
   else
     k_sort_write<true><<<cbk, 256, 0, st>>>(ctx->d_cell_start, ctx->ncell, ctx->d_cell_pid, ctx->d_pos, ctx->d_quat,
                                             ctx->d_cpos, ctx->d_caxis);
-  ctx->launches += 6;
   CU(cudaGetLastError());
   ctx->built = true; ctx->b_seed = seed; ctx->b_step = step;
   return HPMC_OK;
@@ -386,7 +392,6 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
     const uint32_t r = (uint32_t)(((uint64_t)wds[j] * (uint32_t)(i + 1)) >> 32);
     const uint32_t t = perm[i]; perm[i] = perm[r]; perm[r] = t;
   }
-  CU(cudaMemsetAsync(ctx->d_outcome, 0, (size_t)ctx->N, ctx->stream));
 
   MoveArgs a;
   a.g = ctx->g; a.key = key;
