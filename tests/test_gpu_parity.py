@@ -208,3 +208,32 @@ def test_host_buffer_step_matches_device_path():
         assert np.array_equal(hout.numpy(), o.outcomes())
         assert np.array_equal(_bits(hpos.numpy()), _bits(o.pos))
     hh.close(); h.close()
+
+
+@pytest.mark.parametrize("n_c_target", [4, 6, 8])
+def test_small_grids_wrap_rows_and_minimum_image(n_c_target):
+    """Boxes of 4, 6 and 8 cells per axis: every row of the neighbourhood walk wraps for a large share of the cells,
+    the kernel's "no minimum image needed" shortcut is off (n_c = 4), barely on (6) or on for the inner cells (8)."""
+    import dataclasses
+    base = workloads.config("C1")
+    w_min = base.sigma_c + base.sigma_d + 2 * base.d_max
+    L = w_min * (n_c_target + 0.6)
+    N = max(8, int(0.25 * L ** 3 / (np.pi / 6)))
+    cfg = dataclasses.replace(base, N=N, phi_c=N * (np.pi / 6) / L ** 3)
+    pos, _ = workloads.generate(cfg)
+    o, h, dpos, _ = _mk(cfg, pos, None)
+    assert h.n_c == n_c_target == o.n_c
+    h.close()
+    c = run_parity(cfg, pos, None, 60, cfg.n_R(), check_cells_every=5)
+    assert c["rej_depletant"] > 0 and c["rej_hard"] > 0
+
+
+@pytest.mark.parametrize("phi_d", [0.00003, 0.002, 0.6])
+def test_poisson_table_extremes(phi_d):
+    """Tiny and large lambda: a threshold table of a few entries (every guide bucket holds several thresholds or none)
+    and one of ~1300 entries; N_d parity shows up in dep_drawn."""
+    import dataclasses
+    cfg = dataclasses.replace(workloads.config("C3", 4096), phi_d_r=(phi_d,))
+    pos, _ = workloads.generate(cfg)
+    c = run_parity(cfg, pos, None, 12, cfg.n_R())
+    assert c["dep_drawn"] > 0
