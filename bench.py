@@ -35,8 +35,9 @@ BYTES_PER_PARTICLE_PER_PASS = 16.0 # every pass reads the cell-ordered float4 ar
 BYTES_PER_CELL_PER_PASS = 4.0      # ... and each cell_start word once
 BYTES_PER_MOVE = 1.0               # outcome code
 BYTES_PER_ACCEPT = 48.0
-# dram__bytes_read.sum + dram__bytes_write.sum of one move-kernel launch at C3, ncu --set full (profiles/r1b_summary.md)
-NCU_TRAFFIC_BYTES_PER_LAUNCH_C3 = 22.43e6
+# dram__bytes_read.sum + dram__bytes_write.sum of one move-kernel launch at C3, ncu --set full (profiles/r1d_summary.md:
+# 22.50 MB read + 2.8..4.9 MB written)
+NCU_TRAFFIC_BYTES_PER_LAUNCH_C3 = 26.5e6
 LANES_PER_SM_PER_CLK = 128.0       # 4 SMSPs x 32 lanes: issue-rate peak of the plain ALU pipes
 NUM_SMS = 148
 
@@ -121,18 +122,21 @@ def reduce_over_ranks(total_ms, work, device, world):
     return float(t.item()), [float(x) for x in w.tolist()]
 
 
-def oracle_sample(cfg, pos, quat, sweeps, step0):
-    """Time the CPU oracle, as it stands, on `sweeps` sweeps of the same workload with all host cores."""
+def oracle_sample(cfg, pos, quat, sweeps, step0, min_seconds=0.0, max_sweeps=None):
+    """Time the CPU oracle, as it stands, on `sweeps` sweeps of the same workload with all host cores; with
+    min_seconds > 0 keep adding sweeps until that much CPU wall time has been spent (bounded by max_sweeps)."""
     import oracle
     threads = os.cpu_count() or 1
     o = oracle.Oracle(cfg.shape, cfg.sigma_c, cfg.sigma_d, cfg.box_L, cfg.d_max, pos, quat, cfg.disk_a, cfg.disk_s,
                       threads=threads)
     times = []
-    for s in range(sweeps):
+    s = 0
+    while s < sweeps or (sum(times) < min_seconds and (max_sweeps is None or s < max_sweeps)):
         t0 = time.perf_counter()
         o.build_cells(cfg.seed, step0 + s)
         o.sweep(cfg.seed, step0 + s, cfg.n_R(), cfg.d_max, cfg.a_max, cfg.n_trial)
         times.append(time.perf_counter() - t0)
+        s += 1
     c = o.counters()
     return o, c, times, oracle.lib().oracle_get_threads()
 
@@ -293,8 +297,9 @@ def main():
         }
         cpu = None
         if not args.no_cpu_baseline and world == 1:
-            ns = 3 if cfg.N > 200000 else 20
-            _, oc, times, threads = oracle_sample(cfg, pos, quat, ns, args.warmup)
+            # bounded sample: about 12 s of oracle time on this box's cores (3 sweeps at least, 2000 at most)
+            _, oc, times, threads = oracle_sample(cfg, pos, quat, 3, args.warmup, min_seconds=12.0, max_sweeps=2000)
+            ns = len(times)
             om = oc["trials_trans"] + oc["trials_rot"]
             cpu = {"value": om / sum(times), "unit": "moves/s", "cores": threads, "kind": "oracle",
                    "sample": "%d sweeps of the same workload from the same initial poses (%.1f s)" % (ns, sum(times)),
