@@ -201,7 +201,7 @@ int setup_moveq(hpmc_ctx* ctx) {
   const int nact = ctx->ncell / 8;
   const int resident = ctx->num_sms * per_sm;
   int cpc = (nact + resident - 1) / resident;
-  if (cpc < 32) cpc = 32;
+  if (cpc < 8) cpc = 8;   // small systems are latency-bound: more, smaller CTAs (measured on C1, C2, C4)
   if (const char* o = getenv("HPMC_CELLS_PER_CTA")) { const int v = atoi(o); if (v >= 1) cpc = v; }
   constexpr int QM = QCfg<SHAPE>::CPT * QT;
   int nsub = (cpc + QM - 1) / QM;
