@@ -64,7 +64,6 @@ struct hpmc_ctx {
   size_t table_rr = 0;
   int num_sms = 148;
   int move_ctas = 0;
-  unsigned int* d_tiles = nullptr;     // 8 tile counters, one per pass of a sweep
   int q_ctas = 0;                      // CTAs of the item-queue move kernel
   int q_cpc = 0, q_big = 0, q_small = 0;   // active cells per CTA (one wave), tile sizes
   bool use_queue = true;               // HPMC_MOVE_KERNEL=warp selects the first (warp-per-cell) design
@@ -295,7 +294,6 @@ int hpmc_init(hpmc_ctx** out, const hpmc_params* p, int64_t N, float* d_pos4, fl
   CUI(cudaMalloc(&ctx->d_outcome, (size_t)N));
   CUI(cudaMalloc(&ctx->d_counters, sizeof(unsigned long long) * C_COUNT));
   CUI(cudaMalloc(&ctx->d_err, sizeof(int)));
-  CUI(cudaMalloc(&ctx->d_tiles, sizeof(unsigned int) * 8));
   CUI(cudaMemsetAsync(ctx->d_outcome, 0, (size_t)N, ctx->stream));
   CUI(cudaMemsetAsync(ctx->d_counts, 0, sizeof(uint32_t) * ctx->ncell, ctx->stream));   // kept zero between builds by k_scan_apply
   CUI(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * C_COUNT, ctx->stream));
@@ -329,7 +327,7 @@ void hpmc_destroy(hpmc_ctx* ctx) {
   if (ctx->own_pose) { cudaFree(ctx->d_pos); cudaFree(ctx->d_quat); }
   cudaFree(ctx->d_cpos); cudaFree(ctx->d_caxis); cudaFree(ctx->d_cid); cudaFree(ctx->d_rank);
   cudaFree(ctx->d_cell_pid); cudaFree(ctx->d_counts); cudaFree(ctx->d_cell_start); cudaFree(ctx->d_tile_sums);
-  cudaFree(ctx->d_outcome); cudaFree(ctx->d_counters); cudaFree(ctx->d_err); cudaFree(ctx->d_tiles);
+  cudaFree(ctx->d_outcome); cudaFree(ctx->d_counters); cudaFree(ctx->d_err);
   for (auto& t : ctx->tables) { cudaFree(t.d_T); cudaFree(t.d_G); }
   for (auto& e : ctx->ev) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   delete ctx;
