@@ -58,6 +58,9 @@ __device__ __forceinline__ float sym_unit_bits(uint32_t x) {
   return fmaf(f - 1.5f, 2.0f, 1.1920928955078125e-07f);
 }
 
+#ifndef HPMC_WALK_DEFER
+#define HPMC_WALK_DEFER 1
+#endif
 #ifndef HPMC_WALK_SLOTS
 #define HPMC_WALK_SLOTS 4         // phase 1b: particle loads in flight per (move, row) item
 #endif
@@ -94,7 +97,8 @@ struct QSmem {
   static constexpr size_t o_hitems = o_todo + 4 * (M / 32);
   static constexpr size_t o_scal = o_hitems + 4 * HCAP;                         // u32[8]
   static constexpr size_t o_alive = o_scal + 32;                                // u16[M]
-  static constexpr size_t bytes = o_alive + 2 * M;
+  static constexpr size_t o_ovf = o_alive + 2 * M;                              // u32[T] overflow queue of phase 1b
+  static constexpr size_t bytes = o_ovf + 4 * T;
 };
 
 template <int SHAPE>
@@ -143,6 +147,7 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
   constexpr int E = Lq::ENTRY;
   constexpr int M = S::M, POOL = S::POOL, HCAP = S::HCAP, NW = M / 32;
   constexpr int SLOTS = HPMC_WALK_SLOTS;
+  constexpr bool DEFER = HPMC_WALK_DEFER && !ANISO && (9 * M < 65536);   // overflow queue of phase 1b
   const MoveArgs& A = Q.m;
   const Geo& g = A.g;
 
@@ -164,6 +169,7 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
   uint32_t* s_hitems = reinterpret_cast<uint32_t*>(sb_ + S::o_hitems);
   uint32_t* s_scal = reinterpret_cast<uint32_t*>(sb_ + S::o_scal);   // [0] nalive [1] pool top [3] nhard [4] nlist
   uint16_t* s_alive = reinterpret_cast<uint16_t*>(sb_ + S::o_alive);
+  uint32_t* s_ovf = reinterpret_cast<uint32_t*>(sb_ + S::o_ovf);
 
   const int t = threadIdx.x;
   const int nc = g.nc, hc = A.hc;
@@ -182,7 +188,7 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
     const uint32_t tile_n = min((first_tile && (blockIdx.x & 1u)) ? (uint32_t)Q.tile_small : (uint32_t)Q.tile_big, cta_hi - cur);
     const uint32_t tile_lo = cur;
     cur += tile_n; first_tile = false;
-    if (t == 0) { s_scal[0] = 0; s_scal[1] = 0; s_scal[3] = 0; s_scal[4] = 0; }
+    if (t == 0) { s_scal[0] = 0; s_scal[1] = 0; s_scal[3] = 0; s_scal[4] = 0; s_scal[7] = 0; }
     __syncthreads();
 
     // ================================================================ phase 1a: one thread per active cell
@@ -251,8 +257,17 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
     const int nlist = (int)s_scal[4];
 
     // ================================================================ phase 1b: one thread per (move, x-row) item
+    // Two passes over work units: first every item's leading SLOTS particles; an item with more particles in its row
+    // (8 % of the rows at C3, but some lane of nearly every warp) does not make its whole warp loop again: it defers
+    // the rest to an overflow queue, and the second pass spreads those leftovers over all lanes of the CTA.
+    int n_units = nlist * 9;
 #pragma unroll 1
-    for (int it = t; it < nlist * 9; it += T) {
+    for (int pass = 0; pass < 2; ++pass) {
+#pragma unroll 1
+    for (int un = t; un < n_units; un += T) {
+      int it = un;
+      uint32_t i_first = 0;
+      if (pass != 0) { const uint32_t wq = s_ovf[un]; it = (int)(wq & 0xffffu); i_first = wq >> 16; }
       const int e = it / 9, row = it - 9 * e;
       const float4 r1f = s_r1[e];
       const V3 r1 = V3{r1f.x, r1f.y, r1f.z};
@@ -277,7 +292,11 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
       // SLOTS particles in flight per trip (a row holds 2.2 particles on average at C3; more slots cost registers and
       // with them a resident CTA per SM: 4 and 5 measured equal, 6 and 8 slower)
 #pragma unroll 1
-      for (uint32_t i0 = 0; i0 < len; i0 += SLOTS) {
+      for (uint32_t i0 = i_first; i0 < len; i0 += SLOTS) {
+        if (DEFER && pass == 0 && i0 != 0) {
+          const uint32_t qi = atomicAdd(&s_scal[7], 1u);
+          if (qi < (uint32_t)T) { s_ovf[qi] = (uint32_t)it | (i0 << 16); break; }   // queue full: finish inline
+        }
         float4 pj[SLOTS];
 #pragma unroll
         for (int u = 0; u < SLOTS; ++u) {
@@ -312,6 +331,10 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
           }
         }
       }
+    }
+      if (!DEFER) break;
+      __syncthreads();
+      n_units = (int)min(s_scal[7], (uint32_t)T);
     }
     // ================================================================ phase 1c: convex hard-overlap items (a6)
     if (ANISO) {
