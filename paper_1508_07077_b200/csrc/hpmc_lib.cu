@@ -200,6 +200,18 @@ int setup_moveq(hpmc_ctx* ctx) {
   const int nact = ctx->ncell / 8;
   const int resident = ctx->num_sms * per_sm;
   int cpc = (nact + resident - 1) / resident;
+  {
+    // keep the expected number of listed neighbours of a tile within the shared-memory pool (the error flag
+    // HPMC_E_NEIGHBOR_OVERFLOW stays as the backstop): ideal-gas estimate of the neighbours inside the list radius,
+    // times 2 (contact shell of a dense hard-particle fluid or crystal), for every non-empty cell of the tile
+    const double L = ctx->p.box_L, dens = (double)ctx->N / (L * L * L);
+    const double rl = (double)ctx->p.sigma_c + ctx->p.sigma_d + 1e-3;
+    const double nbr = 2.0 * dens * (4.0 * M_PI / 3.0) * rl * rl * rl + 1.0;
+    const double occ = (double)ctx->N / (double)ctx->ncell;
+    const double pmove = occ < 1.0 ? occ : 1.0;
+    const int cap = (int)((double)QSmem<SHAPE, QT, QCfg<SHAPE>::CPT>::POOL / (nbr * pmove));
+    if (cpc > cap) cpc = cap;
+  }
   if (cpc < 8) cpc = 8;   // small systems are latency-bound: more, smaller CTAs (measured on C1, C2, C4)
   if (const char* o = getenv("HPMC_CELLS_PER_CTA")) { const int v = atoi(o); if (v >= 1) cpc = v; }
   constexpr int QM = QCfg<SHAPE>::CPT * QT;

@@ -237,3 +237,13 @@ def test_poisson_table_extremes(phi_d):
     pos, _ = workloads.generate(cfg)
     c = run_parity(cfg, pos, None, 12, cfg.n_R())
     assert c["dep_drawn"] > 0
+
+
+def test_dense_fcc_crystal_neighbour_pool():
+    """A dense fcc crystal (phi = 0.66: 12 neighbours inside the list radius of every move) at a size where the tiles
+    are large: the per-tile neighbour pool must hold (the library reports HPMC_E_NEIGHBOR_OVERFLOW otherwise)."""
+    import dataclasses
+    cfg = dataclasses.replace(workloads.config("C2", 4 * 64 ** 3), phi_c=0.66, q=0.08, d_max=0.03, phi_d_r=(0.1,))
+    pos, _ = workloads.generate(cfg)
+    c = run_parity(cfg, pos, None, 3, cfg.n_R(), check_cells_every=1)
+    assert c["rej_hard"] > 0
