@@ -372,6 +372,7 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
     __syncthreads();
     // ================================================================ phase 2: depletant items (a8)
     if (nalive > 0) {
+      const int nw_alive = (nalive + 31) >> 5;
       int j = t % nalive;
       uint32_t m = s_alive[j];
       uint32_t c_pid = __float_as_uint(s_r1[m].w), c_Nd = s_Nd[m];
@@ -396,9 +397,9 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
             // this move has no unclaimed work left: retire its bit, attach to an unfinished move of the tile
             atomicAnd(&s_todo[j >> 5], ~(1u << (j & 31)));
             int found = -1;
+            int wi = j >> 5;
 #pragma unroll 1
-            for (int i = 0; i < NW; ++i) {
-              const int wi = ((j >> 5) + i) % NW;
+            for (int i = 0; i < nw_alive; ++i) {            // only the words that ever held a bit
               const uint32_t w = v_todo[wi];
               if (w) {
                 const int r = t & 31;
@@ -406,6 +407,7 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
                 found = wi * 32 + ((__ffs(w2) - 1 + r) & 31);
                 break;
               }
+              wi = (wi + 1 == nw_alive) ? 0 : wi + 1;
             }
             if (found < 0) { active = false; break; }
             j = found;
