@@ -475,18 +475,21 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
     __syncthreads();
   }
 
-  // ---- counters: warp reduction, one atomic per warp and counter
+  // ---- counters: hardware warp reduction (REDUX), CTA total in shared memory, one global atomic per CTA and counter
   const unsigned FULL = 0xffffffffu;
-  unsigned long long v[11] = {n_tt, n_at, n_tr, n_ar, n_rb, n_rh, n_rd, n_drawn, n_needed, n_eval, n_blocks};
+  const uint32_t v[11] = {n_tt, n_at, n_tr, n_ar, n_rb, n_rh, n_rd, n_drawn, n_needed, n_eval, n_blocks};
   const int idx[11] = {C_TRIALS_TRANS, C_ACCEPT_TRANS, C_TRIALS_ROT, C_ACCEPT_ROT, C_REJ_BOUNDARY, C_REJ_HARD,
                        C_REJ_DEPLETANT, C_DEP_DRAWN, C_DEP_NEEDED, C_DEP_EVALUATED, C_PHILOX_BLOCKS};
+  unsigned long long* s_cnt = reinterpret_cast<unsigned long long*>(s_r1);     // the tile arrays are dead by now
+  if (t < C_COUNT) s_cnt[t] = 0ull;
+  __syncthreads();
 #pragma unroll
   for (int c = 0; c < 11; ++c) {
-    unsigned long long x = v[c];
-#pragma unroll
-    for (int o = 16; o >= 1; o >>= 1) x += __shfl_xor_sync(FULL, x, o);
-    if ((t & 31) == 0 && x) atomicAdd(&A.counters[idx[c]], x);
+    const uint32_t x = __reduce_add_sync(FULL, v[c]);        // per-warp sums stay far below 2^32
+    if ((t & 31) == 0 && x) atomicAdd(&s_cnt[idx[c]], (unsigned long long)x);
   }
+  __syncthreads();
+  if (t < C_COUNT && s_cnt[t]) atomicAdd(&A.counters[t], s_cnt[t]);
 }
 
 }  // namespace hpmc
