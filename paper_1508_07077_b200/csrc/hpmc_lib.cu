@@ -184,7 +184,10 @@ int get_table(hpmc_ctx* ctx, double lambda, PoissonTable** out) {
 #ifndef HPMC_QCPT
 #define HPMC_QCPT 2
 #endif
-constexpr int QT = 128;                // threads per CTA of the item-queue kernel
+#ifndef HPMC_QT
+#define HPMC_QT 128
+#endif
+constexpr int QT = HPMC_QT;                // threads per CTA of the item-queue kernel
 template <int SHAPE> struct QCfg { static constexpr int CPT = SHAPE == SH_SPHERE ? HPMC_QCPT : 1; };   // tile capacity CPT*QT cells
 
 template <int SHAPE>

@@ -385,7 +385,7 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
       }
       volatile uint32_t* v_rejmin = s_rejmin;
       volatile uint32_t* v_todo = s_todo;
-      uint32_t k = 0, att = 0;
+      uint32_t k = 0, att = 0, trip = 0;
       bool have = false, active = true;
       for (;;) {
         // ---- claim (divergent, short): lanes without an item take the next k of their move, or re-attach
@@ -420,7 +420,8 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
           }
         }
         // the vote is also the reconvergence point: the Philox block below runs with the whole warp together
-        if (!__any_sync(0xffffffffu, active)) break;
+        // (checked every fourth trip: a warp that has run dry idles through at most three cheap trips)
+        if ((++trip & 3u) == 0u && !__any_sync(0xffffffffu, active)) break;
         if (active) {
           // one Philox block = one cube-rejection attempt of depletant k (R-S3)
           const Block4 r = philox(A.key, c_pid, k, 0, c3dep + (att << 16));
@@ -480,16 +481,16 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
   const uint32_t v[11] = {n_tt, n_at, n_tr, n_ar, n_rb, n_rh, n_rd, n_drawn, n_needed, n_eval, n_blocks};
   const int idx[11] = {C_TRIALS_TRANS, C_ACCEPT_TRANS, C_TRIALS_ROT, C_ACCEPT_ROT, C_REJ_BOUNDARY, C_REJ_HARD,
                        C_REJ_DEPLETANT, C_DEP_DRAWN, C_DEP_NEEDED, C_DEP_EVALUATED, C_PHILOX_BLOCKS};
-  unsigned long long* s_cnt = reinterpret_cast<unsigned long long*>(s_r1);     // the tile arrays are dead by now
-  if (t < C_COUNT) s_cnt[t] = 0ull;
+  uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_r1);     // the tile arrays are dead by now; CTA totals stay < 2^32
+  if (t < C_COUNT) s_cnt[t] = 0u;
   __syncthreads();
 #pragma unroll
   for (int c = 0; c < 11; ++c) {
     const uint32_t x = __reduce_add_sync(FULL, v[c]);        // per-warp sums stay far below 2^32
-    if ((t & 31) == 0 && x) atomicAdd(&s_cnt[idx[c]], (unsigned long long)x);
+    if ((t & 31) == 0 && x) atomicAdd(&s_cnt[idx[c]], x);
   }
   __syncthreads();
-  if (t < C_COUNT && s_cnt[t]) atomicAdd(&A.counters[t], s_cnt[t]);
+  if (t < C_COUNT && s_cnt[t]) atomicAdd(&A.counters[t], (unsigned long long)s_cnt[t]);
 }
 
 }  // namespace hpmc
