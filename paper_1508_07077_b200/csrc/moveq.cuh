@@ -3,13 +3,16 @@
 // C3 has 175,616 active cells per pass and a B200 holds ~150k resident threads of this kernel, so a pass is ONE wave
 // of work.  Every phase is spread over all T lanes of the CTA and every dependent-load chain is kept short:
 //   tiling   every CTA owns a contiguous range of active cells, sized by the host so that all CTAs are resident at
-//            once (one wave, no tile counter), and works through it in tiles of <= T cells.
+//            once (one wave, no tile counter), and handles it as one tile of <= CPT*T cells (more tiles only for
+//            systems too large for one wave); C3: 1179 CTAs x 149 cells, ~73 moves per 128 lanes.
 //   phase 1a one THREAD per active cell: pick (a3), trial pose + confinement (a4).  Moves that stay in their cell are
 //            compacted into a dense list in shared memory (empty cells and boundary rejections drop out here).
 //   phase 1b one thread per (move, x-row) item, 9 rows per move: the row's 3 cells are one contiguous span of the
-//            cell-ordered array (two spans when the row wraps); particles are loaded four at a time, the sphere
+//            cell-ordered array (two spans when the row wraps); four particle loads are in flight per item, rows with
+//            more particles hand their rest to an overflow queue that a second pass spreads over all lanes; the sphere
 //            hard-overlap test runs inline (a5, a6), neighbours that a depletant of the move can touch are pushed on
-//            the move's linked list in a CTA-wide shared-memory pool.
+//            the move's linked list in a CTA-wide shared-memory pool.  Moves more than two cells away from the
+//            coordinate wrap skip the minimum image (the plain difference is the minimum image there).
 //   phase 1c (convex shapes) the (move, neighbour) pairs inside the circumsphere distance are items of their own;
 //            the CTA's lanes run the support-function test on them side by side.
 //   phase 1d one thread per move: N_d by table inversion (a7), one 16-byte load instead of an eleven-step binary
