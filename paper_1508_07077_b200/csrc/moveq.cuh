@@ -142,6 +142,91 @@ __device__ __forceinline__ uint32_t poisson_count(const unsigned long long* __re
   return (uint32_t)lo;
 }
 
+// Pointers to the phase-2 tables of one CTA: its own shared memory, or (thread-block clusters) a peer's through
+// distributed shared memory.
+struct QTables {
+  const float4* r1; const float4* rho; const float4* aold; const float4* anew; const float4* pool;
+  const uint32_t* Nd; uint32_t* knext; uint32_t* rejmin; const int* head; uint32_t* todo; const uint16_t* alive;
+};
+
+// Phase 2 (a8): the depletant item queue over the `nalive` surviving moves described by `tb`; returns when no move
+// of the tile has unclaimed work left and this thread's last item is done.
+template <int SHAPE>
+__device__ __forceinline__ void q_depletant_queue(const QTables& tb, int nalive, const Geo& g, const Key10& key,
+                                                  uint32_t c3dep, int t, uint32_t& n_eval, uint32_t& n_blocks) {
+  constexpr bool ANISO = SHAPE != SH_SPHERE;
+  if (nalive <= 0) return;
+  const int nw_alive = (nalive + 31) >> 5;
+  int j = t % nalive;
+  uint32_t m = tb.alive[j];
+  uint32_t c_pid = __float_as_uint(tb.r1[m].w), c_Nd = tb.Nd[m];
+  int c_head = tb.head[m];
+  float4 c_rho = tb.rho[m];
+  V3 c_aold = V3{0.f, 0.f, 1.f}, c_anew = V3{0.f, 0.f, 1.f};
+  if (ANISO) {
+    const float4 ao = tb.aold[m], an = tb.anew[m];
+    c_aold = V3{ao.x, ao.y, ao.z}; c_anew = V3{an.x, an.y, an.z};
+  }
+  volatile uint32_t* v_rejmin = tb.rejmin;
+  volatile uint32_t* v_todo = tb.todo;
+  uint32_t k = 0, att = 0, trip = 0;
+  bool have = false, active = true;
+  for (;;) {
+    // ---- claim (divergent, short): lanes without an item take the next k of their move, or re-attach
+    if (active && !have) {
+#pragma unroll 1
+      for (;;) {
+        k = atomicAdd(&tb.knext[m], 1u);
+        if (k < min(c_Nd, v_rejmin[m])) { att = 0; have = true; break; }
+        // this move has no unclaimed work left: retire its bit, attach to an unfinished move of the tile
+        atomicAnd(&tb.todo[j >> 5], ~(1u << (j & 31)));
+        int found = -1;
+        int wi = j >> 5;
+#pragma unroll 1
+        for (int i = 0; i < nw_alive; ++i) {            // only the words that ever held a bit
+          const uint32_t w = v_todo[wi];
+          if (w) {
+            const int r = t & 31;
+            const uint32_t w2 = __funnelshift_r(w, w, r);
+            found = wi * 32 + ((__ffs(w2) - 1 + r) & 31);
+            break;
+          }
+          wi = (wi + 1 == nw_alive) ? 0 : wi + 1;
+        }
+        if (found < 0) { active = false; break; }
+        j = found;
+        m = tb.alive[j];
+        c_pid = __float_as_uint(tb.r1[m].w); c_Nd = tb.Nd[m]; c_head = tb.head[m]; c_rho = tb.rho[m];
+        if (ANISO) {
+          const float4 ao = tb.aold[m], an = tb.anew[m];
+          c_aold = V3{ao.x, ao.y, ao.z}; c_anew = V3{an.x, an.y, an.z};
+        }
+      }
+    }
+    // the vote is also the reconvergence point: the Philox block below runs with the whole warp together
+    // (checked every fourth trip: a warp that has run dry idles through at most three cheap trips)
+    if ((++trip & 3u) == 0u && !__any_sync(0xffffffffu, active)) break;
+    if (active) {
+      // one Philox block = one cube-rejection attempt of depletant k (R-S3)
+      const Block4 r = philox(key, c_pid, k, 0, c3dep + (att << 16));
+      ++n_blocks;
+      V3 d = V3{g.Rins * sym_unit_bits(r.x), g.Rins * sym_unit_bits(r.y), g.Rins * sym_unit_bits(r.z)};
+      bool inside = dot3(d, d) <= g.Rins2;
+      if (!inside && att == 63u) { d = V3{0.f, 0.f, 0.f}; inside = true; }
+      if (inside) {
+        ++n_eval;
+        const V3 ro = V3{c_rho.x, c_rho.y, c_rho.z};
+        if (q_new_only<SHAPE>(g, d, ro, c_aold, c_anew) && q_free_of_nbrs<SHAPE>(g, tb.pool, c_head, d))
+          atomicMin(&tb.rejmin[m], k);
+        have = false;
+      } else {
+        ++att;
+        if (k > v_rejmin[m]) have = false;     // a lower k already rejects: this one cannot matter
+      }
+    }
+  }
+}
+
 template <int SHAPE, int T, int CPT>
 __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QArgs Q) {
   using Lq = QLayout<SHAPE>;
@@ -374,76 +459,11 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
     }
     __syncthreads();
     // ================================================================ phase 2: depletant items (a8)
-    if (nalive > 0) {
-      const int nw_alive = (nalive + 31) >> 5;
-      int j = t % nalive;
-      uint32_t m = s_alive[j];
-      uint32_t c_pid = __float_as_uint(s_r1[m].w), c_Nd = s_Nd[m];
-      int c_head = s_head[m];
-      float4 c_rho = s_rho[m];
-      V3 c_aold = V3{0.f, 0.f, 1.f}, c_anew = V3{0.f, 0.f, 1.f};
-      if (ANISO) {
-        const float4 ao = s_aold[m], an = s_anew[m];
-        c_aold = V3{ao.x, ao.y, ao.z}; c_anew = V3{an.x, an.y, an.z};
-      }
-      volatile uint32_t* v_rejmin = s_rejmin;
-      volatile uint32_t* v_todo = s_todo;
-      uint32_t k = 0, att = 0, trip = 0;
-      bool have = false, active = true;
-      for (;;) {
-        // ---- claim (divergent, short): lanes without an item take the next k of their move, or re-attach
-        if (active && !have) {
-#pragma unroll 1
-          for (;;) {
-            k = atomicAdd(&s_knext[m], 1u);
-            if (k < min(c_Nd, v_rejmin[m])) { att = 0; have = true; break; }
-            // this move has no unclaimed work left: retire its bit, attach to an unfinished move of the tile
-            atomicAnd(&s_todo[j >> 5], ~(1u << (j & 31)));
-            int found = -1;
-            int wi = j >> 5;
-#pragma unroll 1
-            for (int i = 0; i < nw_alive; ++i) {            // only the words that ever held a bit
-              const uint32_t w = v_todo[wi];
-              if (w) {
-                const int r = t & 31;
-                const uint32_t w2 = __funnelshift_r(w, w, r);
-                found = wi * 32 + ((__ffs(w2) - 1 + r) & 31);
-                break;
-              }
-              wi = (wi + 1 == nw_alive) ? 0 : wi + 1;
-            }
-            if (found < 0) { active = false; break; }
-            j = found;
-            m = s_alive[j];
-            c_pid = __float_as_uint(s_r1[m].w); c_Nd = s_Nd[m]; c_head = s_head[m]; c_rho = s_rho[m];
-            if (ANISO) {
-              const float4 ao = s_aold[m], an = s_anew[m];
-              c_aold = V3{ao.x, ao.y, ao.z}; c_anew = V3{an.x, an.y, an.z};
-            }
-          }
-        }
-        // the vote is also the reconvergence point: the Philox block below runs with the whole warp together
-        // (checked every fourth trip: a warp that has run dry idles through at most three cheap trips)
-        if ((++trip & 3u) == 0u && !__any_sync(0xffffffffu, active)) break;
-        if (active) {
-          // one Philox block = one cube-rejection attempt of depletant k (R-S3)
-          const Block4 r = philox(A.key, c_pid, k, 0, c3dep + (att << 16));
-          ++n_blocks;
-          V3 d = V3{g.Rins * sym_unit_bits(r.x), g.Rins * sym_unit_bits(r.y), g.Rins * sym_unit_bits(r.z)};
-          bool inside = dot3(d, d) <= g.Rins2;
-          if (!inside && att == 63u) { d = V3{0.f, 0.f, 0.f}; inside = true; }
-          if (inside) {
-            ++n_eval;
-            const V3 ro = V3{c_rho.x, c_rho.y, c_rho.z};
-            if (q_new_only<SHAPE>(g, d, ro, c_aold, c_anew) && q_free_of_nbrs<SHAPE>(g, s_pool, c_head, d))
-              atomicMin(&s_rejmin[m], k);
-            have = false;
-          } else {
-            ++att;
-            if (k > v_rejmin[m]) have = false;     // a lower k already rejects: this one cannot matter
-          }
-        }
-      }
+    {
+      QTables tb;
+      tb.r1 = s_r1; tb.rho = s_rho; tb.aold = s_aold; tb.anew = s_anew; tb.pool = s_pool;
+      tb.Nd = s_Nd; tb.knext = s_knext; tb.rejmin = s_rejmin; tb.head = s_head; tb.todo = s_todo; tb.alive = s_alive;
+      q_depletant_queue<SHAPE>(tb, nalive, g, A.key, c3dep, t, n_eval, n_blocks);
     }
     __syncthreads();
     // ================================================================ commit (a10)
