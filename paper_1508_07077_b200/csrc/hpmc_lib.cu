@@ -65,6 +65,7 @@ struct hpmc_ctx {
   int num_sms = 148;
   int move_ctas = 0;
   int q_ctas = 0;                      // CTAs of the item-queue move kernel
+  float q_ramp = 0.0f;                 // work ramp over the CTAs of the move kernel (see moveq.cuh)
   int q_cpc = 0, q_big = 0, q_small = 0;   // active cells per CTA (one wave), tile sizes
   bool use_queue = true;               // HPMC_MOVE_KERNEL=warp selects the first (warp-per-cell) design
   int64_t launches = 0;
@@ -203,6 +204,7 @@ int setup_moveq(hpmc_ctx* ctx) {
   const int nact = ctx->ncell / 8;
   const int resident = ctx->num_sms * per_sm;
   int cpc = (nact + resident - 1) / resident;
+  int pool_cap = 1 << 30;
   {
     // keep the expected number of listed neighbours of a tile within the shared-memory pool (the error flag
     // HPMC_E_NEIGHBOR_OVERFLOW stays as the backstop): ideal-gas estimate of the neighbours inside the list radius,
@@ -212,14 +214,26 @@ int setup_moveq(hpmc_ctx* ctx) {
     const double nbr = 2.0 * dens * (4.0 * M_PI / 3.0) * rl * rl * rl + 1.0;
     const double occ = (double)ctx->N / (double)ctx->ncell;
     const double pmove = occ < 1.0 ? occ : 1.0;
-    const int cap = (int)((double)QSmem<SHAPE, QT, QCfg<SHAPE>::CPT>::POOL / (nbr * pmove));
-    if (cpc > cap) cpc = cap;
+    pool_cap = (int)((double)QSmem<SHAPE, QT, QCfg<SHAPE>::CPT>::POOL / (nbr * pmove));
+    if (cpc > pool_cap) cpc = pool_cap;
   }
   if (cpc < 8) cpc = 8;   // small systems are latency-bound: more, smaller CTAs (measured on C1, C2, C4)
   if (const char* o = getenv("HPMC_CELLS_PER_CTA")) { const int v = atoi(o); if (v >= 1) cpc = v; }
   constexpr int QM = QCfg<SHAPE>::CPT * QT;
-  int nsub = (cpc + QM - 1) / QM;
-  int big = (cpc + nsub - 1) / nsub;
+  // work ramp: only when the pass is one full wave (then every SM holds per_sm CTAs launched in index order)
+  float ramp = 0.0f;
+  if ((nact + cpc - 1) / cpc > resident / 2) {
+    ramp = 0.2f;    // measured at C3: 0 / 0.1 / 0.15 / 0.2 -> 66.7 / 65.3 / 64.2 / 63.7 us per pass
+    if (const char* o = getenv("HPMC_RAMP")) ramp = (float)atof(o);
+    if (ramp < 0.0f) ramp = 0.0f;
+    if (ramp > 0.5f) ramp = 0.5f;
+  }
+  if ((double)cpc * (1.0 + ramp) > (double)pool_cap) cpc = (int)((double)pool_cap / (1.0 + ramp));
+  if (cpc < 8) cpc = 8;
+  ctx->q_ramp = ramp;
+  const int cmax = (int)std::ceil((double)cpc * (1.0 + ramp)) + 1;     // largest share of a CTA
+  int nsub = (cmax + QM - 1) / QM;
+  int big = (cmax + nsub - 1) / nsub;
   if (big > QM) big = QM;
   int small = big;
   if (const char* o = getenv("HPMC_TILE_BIG")) { const int v = atoi(o); if (v >= 1 && v <= QM) big = v; }
@@ -239,7 +253,7 @@ int launch_moveq(hpmc_ctx* ctx, const MoveArgs& a, const PoissonTable* pt) {
   q.magic_hc = ~0ull / (unsigned long long)a.hc + 1ull;   // floor((2^64-1)/hc)+1 == floor(2^64/hc)+1 unless hc | 2^64
   if ((a.hc & (a.hc - 1)) == 0) q.magic_hc = (1ull << 63) / (unsigned long long)a.hc * 2ull + 1ull;
   q.pguide = pt->has_guide ? pt->d_G : nullptr;
-  q.cells_per_cta = ctx->q_cpc; q.tile_big = ctx->q_big; q.tile_small = ctx->q_small;
+  q.ramp = ctx->q_ramp; q.tile_big = ctx->q_big; q.tile_small = ctx->q_small;
   q.wlo = 2.1f * a.g.w; q.whi = a.g.L - 2.1f * a.g.w;
   {
     const float rl = (ctx->p.sigma_c + ctx->p.sigma_d) + 1e-3f;

@@ -45,7 +45,7 @@ struct QArgs {
   unsigned long long magic_hc;     // floor(2^64 / hc) + 1: exact a / hc by __umul64hi for a < 2^32
   const uint4* pguide;             // [4096] guide table of the Poisson thresholds (poisson_count), or nullptr
   float wlo, whi;                  // 2.1 w and L - 2.1 w: centres in between need no minimum image (phase 1b)
-  int cells_per_cta;               // CTA b owns the active cells [b cells_per_cta, (b+1) cells_per_cta)
+  float ramp;                      // share of the first / last CTA relative to the average: 1 + ramp / 1 - ramp
   int tile_big, tile_small;        // ... and works through them in tiles of tile_big <= CPT*T cells; odd CTAs start with
                                    // one tile of tile_small cells (a phase stagger between neighbouring CTAs; measured
                                    // neutral at C3, so the host sets tile_small = tile_big)
@@ -269,8 +269,16 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
   uint32_t n_tt = 0, n_at = 0, n_tr = 0, n_ar = 0, n_rb = 0, n_rh = 0, n_rd = 0;
   uint32_t n_drawn = 0, n_needed = 0, n_eval = 0, n_blocks = 0;
 
-  const uint32_t cta_lo = blockIdx.x * (uint32_t)Q.cells_per_cta;
-  const uint32_t cta_hi = min(cta_lo + (uint32_t)Q.cells_per_cta, (uint32_t)A.nact);
+  // CTA b owns the active cells [lo(b), lo(b+1)), lo(i) = nact (x + ramp x (1 - x)), x = i / gridDim.x: the first CTAs
+  // get (1 + ramp) times the average share, the last ones (1 - ramp) times.  The SM's warp arbitration favours the
+  // CTAs that were launched first; with equal shares the last-launched CTA of every SM ends the pass alone.
+  auto range_lo = [&](uint32_t i) -> uint32_t {
+    const double x = (double)i / (double)gridDim.x;
+    const double v = (double)A.nact * (x + (double)Q.ramp * x * (1.0 - x));
+    return i >= gridDim.x ? (uint32_t)A.nact : min((uint32_t)v, (uint32_t)A.nact);
+  };
+  const uint32_t cta_lo = range_lo(blockIdx.x);
+  const uint32_t cta_hi = range_lo(blockIdx.x + 1u);
   bool first_tile = true;
   for (uint32_t cur = cta_lo; cur < cta_hi;) {
     const uint32_t tile_n = min((first_tile && (blockIdx.x & 1u)) ? (uint32_t)Q.tile_small : (uint32_t)Q.tile_big, cta_hi - cur);
