@@ -66,7 +66,7 @@ struct hpmc_ctx {
   int move_ctas = 0;
   int q_ctas = 0;                      // CTAs of the item-queue move kernel
   float q_ramp = 0.0f;                 // work ramp over the CTAs of the move kernel (see moveq.cuh)
-  int q_cpc = 0, q_big = 0, q_small = 0;   // active cells per CTA (one wave), tile sizes
+  int q_cpc = 0, q_big = 0;            // average active cells per CTA (one wave), tile size
   bool use_queue = true;               // HPMC_MOVE_KERNEL=warp selects the first (warp-per-cell) design
   int64_t launches = 0;
   bool timing = false;
@@ -235,14 +235,12 @@ int setup_moveq(hpmc_ctx* ctx) {
   int nsub = (cmax + QM - 1) / QM;
   int big = (cmax + nsub - 1) / nsub;
   if (big > QM) big = QM;
-  int small = big;
   if (const char* o = getenv("HPMC_TILE_BIG")) { const int v = atoi(o); if (v >= 1 && v <= QM) big = v; }
-  if (const char* o = getenv("HPMC_TILE_SMALL")) { const int v = atoi(o); if (v >= 1 && v <= QM) small = v; }
-  ctx->q_cpc = cpc; ctx->q_big = big; ctx->q_small = small;
+  ctx->q_cpc = cpc; ctx->q_big = big;
   ctx->q_ctas = (nact + cpc - 1) / cpc;
   if (getenv("HPMC_VERBOSE"))
-    fprintf(stderr, "k_moveq<%d,%d>: smem %zu B, %d CTAs/SM, %d CTAs x %d cells, tiles %d (odd CTAs start with %d)\n", SHAPE,
-            QT, smem, per_sm, ctx->q_ctas, cpc, big, small);
+    fprintf(stderr, "k_moveq<%d,%d>: smem %zu B, %d CTAs/SM, %d CTAs x %d cells on average (ramp %.2f), tiles of %d\n", SHAPE,
+            QT, smem, per_sm, ctx->q_ctas, cpc, (double)ramp, big);
   return 0;
 }
 
@@ -253,7 +251,7 @@ int launch_moveq(hpmc_ctx* ctx, const MoveArgs& a, const PoissonTable* pt) {
   q.magic_hc = ~0ull / (unsigned long long)a.hc + 1ull;   // floor((2^64-1)/hc)+1 == floor(2^64/hc)+1 unless hc | 2^64
   if ((a.hc & (a.hc - 1)) == 0) q.magic_hc = (1ull << 63) / (unsigned long long)a.hc * 2ull + 1ull;
   q.pguide = pt->has_guide ? pt->d_G : nullptr;
-  q.ramp = ctx->q_ramp; q.tile_big = ctx->q_big; q.tile_small = ctx->q_small;
+  q.ramp = ctx->q_ramp; q.tile_cells = ctx->q_big;
   q.wlo = 2.1f * a.g.w; q.whi = a.g.L - 2.1f * a.g.w;
   {
     const float rl = (ctx->p.sigma_c + ctx->p.sigma_d) + 1e-3f;

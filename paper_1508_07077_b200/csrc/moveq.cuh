@@ -46,9 +46,7 @@ struct QArgs {
   const uint4* pguide;             // [4096] guide table of the Poisson thresholds (poisson_count), or nullptr
   float wlo, whi;                  // 2.1 w and L - 2.1 w: centres in between need no minimum image (phase 1b)
   float ramp;                      // share of the first / last CTA relative to the average: 1 + ramp / 1 - ramp
-  int tile_big, tile_small;        // ... and works through them in tiles of tile_big <= CPT*T cells; odd CTAs start with
-                                   // one tile of tile_small cells (a phase stagger between neighbouring CTAs; measured
-                                   // neutral at C3, so the host sets tile_small = tile_big)
+  int tile_cells;                  // a CTA works through its share in tiles of tile_cells <= CPT*T cells (normally one)
   float rlist2;                    // neighbours farther than this from the new centre cannot touch any depletant
                                    // of the move: (sigma_c + sigma_d + 1e-3)^2 for the plain rule (insertion
                                    // sphere about the new centre only), r_cut^2 of R-3.4 otherwise
@@ -279,11 +277,10 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
   };
   const uint32_t cta_lo = range_lo(blockIdx.x);
   const uint32_t cta_hi = range_lo(blockIdx.x + 1u);
-  bool first_tile = true;
   for (uint32_t cur = cta_lo; cur < cta_hi;) {
-    const uint32_t tile_n = min((first_tile && (blockIdx.x & 1u)) ? (uint32_t)Q.tile_small : (uint32_t)Q.tile_big, cta_hi - cur);
+    const uint32_t tile_n = min((uint32_t)Q.tile_cells, cta_hi - cur);
     const uint32_t tile_lo = cur;
-    cur += tile_n; first_tile = false;
+    cur += tile_n;
     if (t == 0) { s_scal[0] = 0; s_scal[1] = 0; s_scal[3] = 0; s_scal[4] = 0; s_scal[7] = 0; }
     __syncthreads();
 
