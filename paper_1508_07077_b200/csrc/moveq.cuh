@@ -99,7 +99,8 @@ struct QSmem {
   static constexpr size_t o_scal = o_hitems + 4 * HCAP;                         // u32[8]
   static constexpr size_t o_alive = o_scal + 32;                                // u16[M]
   static constexpr size_t o_ovf = o_alive + 2 * M;                              // u32[T] overflow queue of phase 1b
-  static constexpr size_t bytes = o_ovf + 4 * T;
+  static constexpr size_t o_cnt = o_ovf + 4 * T;                                // u32[16] CTA totals of the counters
+  static constexpr size_t bytes = o_cnt + 64;
 };
 
 template <int SHAPE>
@@ -256,6 +257,7 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
   uint32_t* s_scal = reinterpret_cast<uint32_t*>(sb_ + S::o_scal);   // [0] nalive [1] pool top [3] nhard [4] nlist
   uint16_t* s_alive = reinterpret_cast<uint16_t*>(sb_ + S::o_alive);
   uint32_t* s_ovf = reinterpret_cast<uint32_t*>(sb_ + S::o_ovf);
+  uint32_t* s_cnt = reinterpret_cast<uint32_t*>(sb_ + S::o_cnt);
 
   const int t = threadIdx.x;
   const int nc = g.nc, hc = A.hc;
@@ -264,8 +266,10 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
   const uint32_t c3dep = P_DEPPOS + colw;
 
   // per-thread counters (reduced once at the end of the kernel)
-  uint32_t n_tt = 0, n_at = 0, n_tr = 0, n_ar = 0, n_rb = 0, n_rh = 0, n_rd = 0;
-  uint32_t n_drawn = 0, n_needed = 0, n_eval = 0, n_blocks = 0;
+  // counters: the two that tick in the hot loop live in registers; the per-move ones go straight to CTA totals in
+  // shared memory (CTA totals stay far below 2^32), so that they do not occupy registers across phase 2
+  uint32_t n_eval = 0, n_blocks = 0;
+  if (t < C_COUNT) s_cnt[t] = 0u;               // ordered before the first use by the barrier at the top of the tile loop
 
   // CTA b owns the active cells [lo(b), lo(b+1)), lo(i) = nact (x + ramp x (1 - x)), x = i / gridDim.x: the first CTAs
   // get (1 + ramp) times the average share, the last ones (1 - ramp) times.  The SM's warp arbitration favours the
@@ -313,16 +317,16 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
           if (!rot) {
             r1 = V3{wrap1(g, r0.x + A.d_max * sym_unit_bits(rm.x)), wrap1(g, r0.y + A.d_max * sym_unit_bits(rm.y)),
                     wrap1(g, r0.z + A.d_max * sym_unit_bits(rm.z))};
-            ++n_tt;
+            atomicAdd(&s_cnt[C_TRIALS_TRANS], 1u);
           } else {
             const V3 v = ball_sample(A.key, pid, 0, 0, P_MOVE + colw + (1u << 16), A.a_max, A.a_max2, n_blocks);
             q1 = rotate_cayley(q0, v);
-            ++n_tr;
+            atomicAdd(&s_cnt[C_TRIALS_ROT], 1u);
           }
           const int jx = cell_axis(g, r1.x, A.sx), jy = cell_axis(g, r1.y, A.sy), jz = cell_axis(g, r1.z, A.sz);
           if (jx != ix || jy != iy || jz != iz) {        // confinement (L180)
             A.outcome[pid] = (uint8_t)OUT_BOUNDARY;
-            ++n_rb;
+            atomicAdd(&s_cnt[C_REJ_BOUNDARY], 1u);
           } else {
             const uint32_t e = atomicAdd(&s_scal[4], 1u);
             s_r1[e] = make_float4(r1.x, r1.y, r1.z, p0.w);
@@ -482,8 +486,8 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
         const uint32_t Nd = s_Nd[e], rm_ = s_rejmin[e];
         const bool rej = rm_ < Nd;
         out = rej ? OUT_DEPLETANT : OUT_ACCEPT;
-        n_drawn += Nd;
-        n_needed += rej ? rm_ + 1u : Nd;
+        atomicAdd(&s_cnt[C_DEP_DRAWN], Nd);
+        atomicAdd(&s_cnt[C_DEP_NEEDED], rej ? rm_ + 1u : Nd);
       }
       A.outcome[pid] = (uint8_t)out;
       if (out == OUT_ACCEPT) {
@@ -497,25 +501,20 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
           const float4 an = s_anew[e];
           A.caxis[slot] = make_float4(an.x, an.y, an.z, 0.0f);
         }
-        if (rot) ++n_ar; else ++n_at;
-      } else if (out == OUT_HARD) ++n_rh;
-      else ++n_rd;
+        atomicAdd(&s_cnt[rot ? C_ACCEPT_ROT : C_ACCEPT_TRANS], 1u);
+      } else atomicAdd(&s_cnt[out == OUT_HARD ? C_REJ_HARD : C_REJ_DEPLETANT], 1u);
     }
     __syncthreads();
   }
 
-  // ---- counters: hardware warp reduction (REDUX), CTA total in shared memory, one global atomic per CTA and counter
-  const unsigned FULL = 0xffffffffu;
-  const uint32_t v[11] = {n_tt, n_at, n_tr, n_ar, n_rb, n_rh, n_rd, n_drawn, n_needed, n_eval, n_blocks};
-  const int idx[11] = {C_TRIALS_TRANS, C_ACCEPT_TRANS, C_TRIALS_ROT, C_ACCEPT_ROT, C_REJ_BOUNDARY, C_REJ_HARD,
-                       C_REJ_DEPLETANT, C_DEP_DRAWN, C_DEP_NEEDED, C_DEP_EVALUATED, C_PHILOX_BLOCKS};
-  uint32_t* s_cnt = reinterpret_cast<uint32_t*>(s_r1);     // the tile arrays are dead by now; CTA totals stay < 2^32
-  if (t < C_COUNT) s_cnt[t] = 0u;
-  __syncthreads();
-#pragma unroll
-  for (int c = 0; c < 11; ++c) {
-    const uint32_t x = __reduce_add_sync(FULL, v[c]);        // per-warp sums stay far below 2^32
-    if ((t & 31) == 0 && x) atomicAdd(&s_cnt[idx[c]], x);
+  // ---- counters: REDUX for the two register counters, then one global atomic per CTA and counter
+  {
+    const unsigned FULL = 0xffffffffu;
+    const uint32_t xe = __reduce_add_sync(FULL, n_eval), xb = __reduce_add_sync(FULL, n_blocks);
+    if ((t & 31) == 0) {
+      if (xe) atomicAdd(&s_cnt[C_DEP_EVALUATED], xe);
+      if (xb) atomicAdd(&s_cnt[C_PHILOX_BLOCKS], xb);
+    }
   }
   __syncthreads();
   if (t < C_COUNT && s_cnt[t]) atomicAdd(&A.counters[t], (unsigned long long)s_cnt[t]);
