@@ -247,3 +247,17 @@ def test_dense_fcc_crystal_neighbour_pool():
     pos, _ = workloads.generate(cfg)
     c = run_parity(cfg, pos, None, 3, cfg.n_R(), check_cells_every=1)
     assert c["rej_hard"] > 0
+
+
+
+@pytest.mark.parametrize("cells_per_cta,tile", [(600, 64), (280, None)])
+def test_several_tiles_per_cta(monkeypatch, cells_per_cta, tile):
+    """The multi-tile loop of the move kernel is only reached by systems larger than one wave (> ~2.4 M spheres);
+    force it at C3's size: 600 cells per CTA in tiles of 64, and 280 cells per CTA with the work ramp (shares of up to
+    336 cells, two tiles)."""
+    monkeypatch.setenv("HPMC_CELLS_PER_CTA", str(cells_per_cta))
+    if tile:
+        monkeypatch.setenv("HPMC_TILE_BIG", str(tile))
+    cfg = workloads.config("C3")
+    pos, _ = workloads.generate(cfg)
+    run_parity(cfg, pos, None, 2, cfg.n_R(), check_cells_every=1)
