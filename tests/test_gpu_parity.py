@@ -250,14 +250,14 @@ def test_dense_fcc_crystal_neighbour_pool():
 
 
 
-@pytest.mark.parametrize("cells_per_cta,tile", [(600, 64), (280, None)])
+@pytest.mark.parametrize("cells_per_cta,tile", [(600, 64), (None, 64)])
 def test_several_tiles_per_cta(monkeypatch, cells_per_cta, tile):
     """The multi-tile loop of the move kernel is only reached by systems larger than one wave (> ~2.4 M spheres);
-    force it at C3's size: 600 cells per CTA in tiles of 64, and 280 cells per CTA with the work ramp (shares of up to
-    336 cells, two tiles)."""
-    monkeypatch.setenv("HPMC_CELLS_PER_CTA", str(cells_per_cta))
-    if tile:
-        monkeypatch.setenv("HPMC_TILE_BIG", str(tile))
+    force it at C3's size with tiles of 64 cells: fewer, larger CTA shares without the work ramp (the request for 600
+    cells is cut to the neighbour-pool bound, ~180), and the default shares with the ramp (up to ~180 cells)."""
+    if cells_per_cta:
+        monkeypatch.setenv("HPMC_CELLS_PER_CTA", str(cells_per_cta))
+    monkeypatch.setenv("HPMC_TILE_BIG", str(tile))
     cfg = workloads.config("C3")
     pos, _ = workloads.generate(cfg)
     run_parity(cfg, pos, None, 2, cfg.n_R(), check_cells_every=1)
