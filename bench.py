@@ -35,9 +35,9 @@ BYTES_PER_PARTICLE_PER_PASS = 16.0 # every pass reads the cell-ordered float4 ar
 BYTES_PER_CELL_PER_PASS = 4.0      # ... and each cell_start word once
 BYTES_PER_MOVE = 1.0               # outcome code
 BYTES_PER_ACCEPT = 48.0
-# dram__bytes_read.sum + dram__bytes_write.sum of one move-kernel launch at C3, ncu --set full (profiles/r1d_summary.md:
-# 22.50 MB read + 2.8..4.9 MB written)
-NCU_TRAFFIC_BYTES_PER_LAUNCH_C3 = 26.5e6
+# dram__bytes_read.sum + dram__bytes_write.sum of one move-kernel launch at C3, ncu --set full (profiles/r1f_summary.md:
+# 22.50 MB read + 0 written; capture d saw 2.8..4.9 MB of write-backs of the preceding build on top)
+NCU_TRAFFIC_BYTES_PER_LAUNCH_C3 = 22.5e6
 LANES_PER_SM_PER_CLK = 128.0       # 4 SMSPs x 32 lanes: issue-rate peak of the plain ALU pipes
 NUM_SMS = 148
 
