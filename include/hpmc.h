@@ -146,6 +146,22 @@ int64_t hpmc_launch_count(hpmc_ctx* ctx);
 int hpmc_time_move_kernel(hpmc_ctx* ctx, int32_t enable);
 int hpmc_move_kernel_ms(hpmc_ctx* ctx, double* ms_total, int64_t* launches);
 
+/* Micro-benchmark of the plain ALU pipes on the current device (the roofline denominator of the move kernel;
+ * MEASURED_PEAKS.json holds no ALU figure).  rate[i] = thread-instructions per SM per clock of a
+ * dependency-free stream of one kind, 32 resident warps per SM, counted with clock64() (clock-independent):
+ *   [0] FADD  [1] FMUL  [2] FFMA (context: the path is compiled without contraction)  [3] IMAD
+ *   [4] IMAD.WIDE.U32 + LOP3 pairs (one half of a Philox round; both instructions counted)
+ *   [5] LOP3  [6] FADD and LOP3 alternating (both pipes: the issue limit)
+ *   [7],[8],[9] Philox4x32-10 BLOCKS per SM per clock with 1, 2, 4 independent blocks per thread.
+ * out is host memory; needs no context; synchronises cuda_stream.  Takes a few milliseconds. */
+typedef struct {
+  int32_t num_sms;         /* cudaDevAttrMultiProcessorCount */
+  int32_t sm_clock_khz;    /* cudaDevAttrClockRate (nominal maximum) */
+  double sm_mhz_during;    /* SM clock seen during the FADD stream: cycles / event time */
+  double rate[10];
+} hpmc_alu_peaks_t;
+int hpmc_alu_peaks(hpmc_alu_peaks_t* out, void* cuda_stream);
+
 /* Message of the last error on this context (or of the last failed hpmc_init if ctx is NULL). */
 const char* hpmc_last_error(hpmc_ctx* ctx);
 

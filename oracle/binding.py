@@ -84,6 +84,7 @@ def lib() -> C.CDLL:
                 "oracle_cells": (i32, [vp, vp, vp, vp]),
                 "oracle_run": (i32, [vp, u32, u32, i64, f64, f32, f32, i32, vp, vp]),
                 "oracle_eval_move": (i32, [vp, u32, u32, i64, vp, vp, f64, i32]),
+                "oracle_eval_moves": (i32, [vp, u32, u32, i64, i64, vp, vp, f64, i32, vp]),
                 "oracle_count_overlaps": (i64, [vp, i32]),
                 "oracle_philox4x32_10": (None, [vp, vp, vp]),
                 "oracle_unit01": (f32, [u32]),
@@ -187,6 +188,16 @@ class Oracle:
         p = np.ascontiguousarray(pos3, np.float32)
         q = None if quat4 is None else np.ascontiguousarray(quat4, np.float32)
         return self.L.oracle_eval_move(self.h, seed, draw, i, _ptr(p), _ptr(q), float(n_R), n_trial)
+
+    def eval_moves(self, seed, draw0, n, i, pos3, quat4, n_R, n_trial=0):
+        """Outcome codes of n independent evaluations (draw0 .. draw0+n-1) of the same prescribed move."""
+        p = np.ascontiguousarray(pos3, np.float32)
+        q = None if quat4 is None else np.ascontiguousarray(quat4, np.float32)
+        out = np.empty(n, np.uint8)
+        rc = self.L.oracle_eval_moves(self.h, seed, draw0, n, i, _ptr(p), _ptr(q), float(n_R), n_trial, _ptr(out))
+        if rc:
+            raise RuntimeError("oracle_eval_moves rc=%d" % rc)
+        return out
 
     def count_overlaps(self, both_ways=True):
         return int(self.L.oracle_count_overlaps(self.h, 1 if both_ways else 0))

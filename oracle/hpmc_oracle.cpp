@@ -669,6 +669,29 @@ int oracle_eval_move(void* h, uint32_t seed, uint32_t draw, int64_t i, const flo
   return evaluate_move(*c, seed, draw, 0, i, own, r0, q0, r1, q1, n_trial, cn);
 }
 
+// Batched form of oracle_eval_move for the statistical pins: out[j] = oracle_eval_move(h, seed, draw0 + j, ...) for
+// j = 0..n-1.  A plain loop over the same evaluate_move (draws are independent random streams, so the optional
+// OpenMP loop changes nothing); no arithmetic of its own.
+int oracle_eval_moves(void* h, uint32_t seed, uint32_t draw0, int64_t n, int64_t i, const float* pos3,
+                      const float* quat4, double n_R, int32_t n_trial, uint8_t* out) {
+  Ctx* c = (Ctx*)h;
+  if (!c->built) return -3;
+  const double lambda = lambda_of(c->g, n_R);
+  if (c->pt.lambda != lambda) build_poisson(c->pt, lambda);
+  const V3 r0 = load_r(*c, i); const Q4 q0 = load_q(*c, i);
+  const V3 r1 = V3{pos3[0], pos3[1], pos3[2]};
+  const Q4 q1 = quat4 ? Q4{quat4[0], quat4[1], quat4[2], quat4[3]} : q0;
+  const int64_t own = cell_of(*c, r0);
+  const bool outside = cell_of(*c, r1) != own;
+#pragma omp parallel for schedule(static)
+  for (int64_t j = 0; j < n; ++j) {
+    Counters cn;
+    out[j] = outside ? (uint8_t)OUT_BOUNDARY
+                     : (uint8_t)evaluate_move(*c, seed, draw0 + (uint32_t)j, 0, i, own, r0, q0, r1, q1, n_trial, cn);
+  }
+  return 0;
+}
+
 // Number of overlapping pairs (i<j) under the fp32 hard-overlap predicate, evaluated with i as
 // the "mover" and, if both_ways != 0, also requiring the predicate with j as the mover.  Check 1.
 int64_t oracle_count_overlaps(void* h, int32_t both_ways) {

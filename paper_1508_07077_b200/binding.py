@@ -21,6 +21,7 @@ EXPORTS = (
     "hpmc_init", "hpmc_destroy", "hpmc_build_cells", "hpmc_sweep", "hpmc_run", "hpmc_counters",
     "hpmc_reset_counters", "hpmc_outcomes", "hpmc_grid", "hpmc_cells", "hpmc_upload", "hpmc_download",
     "hpmc_step_host", "hpmc_launch_count", "hpmc_time_move_kernel", "hpmc_move_kernel_ms", "hpmc_last_error",
+    "hpmc_alu_peaks",
 )
 
 
@@ -39,6 +40,16 @@ class Params(C.Structure):
 class Counters(C.Structure):
     """hpmc_counters_t"""
     _fields_ = [(n, C.c_uint64) for n in COUNTER_NAMES]
+
+
+ALU_KINDS = ("fadd", "fmul", "ffma", "imad", "imadwide_lop3_pair", "lop3", "fadd_lop3_mix", "philox_blocks_ilp1", "philox_blocks_ilp2",
+             "philox_blocks_ilp4")
+
+
+class AluPeaks(C.Structure):
+    """hpmc_alu_peaks_t"""
+    _fields_ = [("num_sms", C.c_int32), ("sm_clock_khz", C.c_int32), ("sm_mhz_during", C.c_double),
+                ("rate", C.c_double * 10)]
 
 
 def library_path() -> str:
@@ -76,6 +87,7 @@ def load_library() -> C.CDLL:
         "hpmc_time_move_kernel": (i32, [vp, i32]),
         "hpmc_move_kernel_ms": (i32, [vp, P(f64), P(i64)]),
         "hpmc_last_error": (C.c_char_p, [vp]),
+        "hpmc_alu_peaks": (i32, [P(AluPeaks), vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -83,6 +95,20 @@ def load_library() -> C.CDLL:
         fn.argtypes = args
     _LIB = L
     return L
+
+
+def alu_peaks(stream=None):
+    """hpmc_alu_peaks: measured per-SM-per-clock rates of the plain ALU pipes on the current device."""
+    import torch
+    L = load_library()
+    s = torch.cuda.current_stream() if stream is None else stream
+    out = AluPeaks()
+    rc = L.hpmc_alu_peaks(C.byref(out), C.c_void_p(s.cuda_stream))
+    if rc:
+        raise HPMCError(rc, (L.hpmc_last_error(None) or b"").decode())
+    d = {"num_sms": out.num_sms, "sm_clock_khz": out.sm_clock_khz, "sm_mhz_during": out.sm_mhz_during}
+    d.update({k: out.rate[i] for i, k in enumerate(ALU_KINDS)})
+    return d
 
 
 def _dptr(t):

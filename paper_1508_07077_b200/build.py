@@ -11,7 +11,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "hpmc_lib.cu")
-DEPS = [os.path.join(HERE, "csrc", f) for f in ("hpmc_lib.cu", "move.cuh", "moveq.cuh", "cells.cuh", "geometry.cuh", "philox.cuh")]
+DEPS = [os.path.join(HERE, "csrc", f) for f in ("hpmc_lib.cu", "move.cuh", "moveq.cuh", "cells.cuh", "geometry.cuh", "philox.cuh", "alu_peak.cuh")]
 DEPS.append(os.path.join(os.path.dirname(HERE), "include", "hpmc.h"))
 SO = os.path.join(HERE, "libhpmc_b200.so")
 

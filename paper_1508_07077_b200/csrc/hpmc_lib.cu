@@ -16,6 +16,7 @@
 #include <vector>
 
 #include "../../include/hpmc.h"
+#include "alu_peak.cuh"
 #include "cells.cuh"
 #include "move.cuh"
 #include "moveq.cuh"
@@ -570,6 +571,60 @@ int hpmc_move_kernel_ms(hpmc_ctx* ctx, double* ms_total, int64_t* launches) {
   ctx->ev_launches += 8 * (int64_t)ctx->ev_used;
   ctx->ev_used = 0;
   *ms_total = ctx->ev_ms; *launches = ctx->ev_launches;
+  return HPMC_OK;
+}
+
+int hpmc_alu_peaks(hpmc_alu_peaks_t* out, void* cuda_stream) {
+  hpmc_ctx* ctx = nullptr;
+  if (!out) return fail(nullptr, HPMC_E_BADARG, "hpmc_alu_peaks: NULL argument");
+  std::memset(out, 0, sizeof(*out));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int dev = 0, sms = 0, khz = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+    return fail(nullptr, HPMC_E_CUDA, std::string("hpmc_alu_peaks: no usable CUDA device: ") + cudaGetErrorString(cudaGetLastError()));
+  cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev);
+  out->num_sms = sms; out->sm_clock_khz = khz;
+  const int grid = 2 * sms;                       // 2 CTAs x 512 threads = 32 warps per SM, one wave
+  unsigned long long* d_cyc = nullptr;
+  uint32_t* d_sink = nullptr;
+  CU(cudaMalloc(&d_cyc, sizeof(unsigned long long) * grid));
+  CU(cudaMalloc(&d_sink, sizeof(uint32_t)));
+  cudaEvent_t e0, e1;
+  CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+  const Key10 key = make_key(1u, 2u);
+  std::vector<unsigned long long> cyc((size_t)grid);
+  const int iters = 2048;
+  double mhz_sum = 0.0;
+  for (int kind = 0; kind < AK_COUNT; ++kind) {
+    double best = 0.0;
+    for (int rep = 0; rep < 3; ++rep) {           // first repetition warms up the instruction cache
+      CU(cudaMemsetAsync(d_cyc, 0, sizeof(unsigned long long) * grid, st));
+      CU(cudaEventRecord(e0, st));
+#define HPMC_AK(K) case K: k_alu_peak<K><<<grid, AK_THREADS, 0, st>>>(iters, 0x9E3779B9u + rep, 0xBB67AE85u, 1.0000001f, 0.99999994f, key, d_cyc, d_sink); break;
+      switch (kind) {
+        HPMC_AK(AK_FADD) HPMC_AK(AK_FMUL) HPMC_AK(AK_FFMA) HPMC_AK(AK_IMAD) HPMC_AK(AK_IMADW_XOR) HPMC_AK(AK_LOP3) HPMC_AK(AK_MIX)
+        HPMC_AK(AK_PHILOX1) HPMC_AK(AK_PHILOX2) HPMC_AK(AK_PHILOX4)
+      }
+#undef HPMC_AK
+      CU(cudaEventRecord(e1, st));
+      CU(cudaMemcpyAsync(cyc.data(), d_cyc, sizeof(unsigned long long) * grid, cudaMemcpyDeviceToHost, st));
+      CU(cudaStreamSynchronize(st));
+      CU(cudaGetLastError());
+      unsigned long long cmax = 0;
+      for (int i = 0; i < grid; ++i) cmax = cyc[(size_t)i] > cmax ? cyc[(size_t)i] : cmax;
+      float ms = 0.0f;
+      CU(cudaEventElapsedTime(&ms, e0, e1));
+      // thread-instructions per SM per clock: 1024 threads per SM, per thread iters x (32 plain ops | NB Philox blocks)
+      const double per_thread = kind >= AK_PHILOX1 ? (double)iters * (kind == AK_PHILOX1 ? 1.0 : kind == AK_PHILOX2 ? 2.0 : 4.0)
+                                                   : (double)iters * (kind == AK_IMADW_XOR ? 64.0 : 32.0);
+      const double rate = cmax ? 2.0 * AK_THREADS * per_thread / (double)cmax : 0.0;
+      if (rep > 0 && rate > best) { best = rate; if (kind == AK_FADD && ms > 0.0f) mhz_sum = (double)cmax / ((double)ms * 1e3); }
+    }
+    out->rate[kind] = best;
+  }
+  out->sm_mhz_during = mhz_sum;
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  cudaFree(d_cyc); cudaFree(d_sink);
   return HPMC_OK;
 }
 

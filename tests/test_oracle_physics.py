@@ -293,17 +293,125 @@ def test_cb_isolated_colloid_always_accepts_with_many_trials():
     assert (outp[:, 0] == 1).sum() < 0.2 * nb
 
 
-def test_cb_two_sphere_fixed_move_ratio():
-    """CB (n_trial=4) samples the same AO weight: acc(r->r')/acc(r'->r) = exp(n_R [V_ov(r') - V_ov(r)]),
-    up to the <~1-2 % residual of the paper's normalised Eq. 16 documented in DESIGN.md (reading G1)."""
-    cfg = workloads.config("C1")
-    n_R, R, nd = cfg.n_R(), 0.6, 250000
-    ra, rb = 1.05, 1.12
-    fwd, rev = _pair_ratio(n_R, cfg.sigma_d, ra, rb, nd, n_trial=4)
+def _pair_counts(L_, ra, rb, nd, n_trial, n_R, sigma_d, seed=7):
+    """Accepted counts of the fixed move r_a -> r_b and of its reverse (sphere 0 moved along x towards / away from the
+    fixed sphere 1), nd independent evaluations each, through the batched export oracle_eval_moves of library L_."""
+    import ctypes as C
+    from oracle import binding
+    acc = []
+    L_.oracle_set_threads(os.cpu_count() or 1)     # draws are independent streams: the thread count changes no bit
+    for r0, r1 in ((ra, rb), (rb, ra)):
+        p4 = np.zeros((2, 4), np.float32)
+        p4[0, :3] = [3.0 + (2.0 - r0), 4.0, 4.0]
+        p4[1, :3] = [5.0, 4.0, 4.0]
+        par = binding.make_params("sphere", 1.0, sigma_d, 8.0, 0.1)
+        h = L_.oracle_create(C.byref(par), 2, p4.ctypes.data_as(C.c_void_p), None)
+        assert h
+        assert L_.oracle_build_cells(h, 1, 0) == 0
+        new = np.array([3.0 + (2.0 - r1), 4.0, 4.0], np.float32)
+        out = np.empty(nd, np.uint8)
+        rc = L_.oracle_eval_moves(h, seed, 0, nd, 0, new.ctypes.data_as(C.c_void_p), None, float(n_R), n_trial,
+                                  out.ctypes.data_as(C.c_void_p))
+        assert rc == 0
+        assert set(np.unique(out)) <= ({1, 4} if n_trial == 0 else {1, 5})
+        acc.append(int((out == 1).sum()))
+        L_.oracle_destroy(h)
+    L_.oracle_set_threads(1)
+    return acc
+
+
+def _ratio_error(L_, ra, rb, nd, n_trial, n_R, sigma_d):
+    """(measured fwd/rev acceptance ratio) / exp(n_R [V_ov(r_b) - V_ov(r_a)]) - 1, and its 1-sigma statistical error.
+    The target is detailed balance w.r.t. the Asakura-Oosawa weight (ref. 17 L276; Eq. 8 L105 / Eq. 15)."""
+    R = 0.5 * (1.0 + sigma_d)
+    fwd, rev = _pair_counts(L_, ra, rb, nd, n_trial, n_R, sigma_d)
     want = math.exp(n_R * (lens(R, rb) - lens(R, ra)))
-    got = fwd / rev
-    rel = math.sqrt(1 / fwd + 1 / rev)
-    assert abs(got / want - 1) < 3.0 * rel + 0.02, (got, want, fwd, rev)
+    return (fwd / max(rev, 1)) / want - 1.0, math.sqrt(1.0 / max(fwd, 1) + 1.0 / max(rev, 1)), fwd, rev
+
+
+# Geometry of the Eq. 16 pins: C1's depletants (sigma_d = 0.2, n_R = 47.7), sphere 0 moved from separation 1.02 to 1.10
+# from a fixed neighbour.  The old-only crescent faces the neighbour and is partly covered by its exclusion sphere,
+# the new-only crescent faces away and is free: the forward and reverse success fractions of Eq. 16 differ (s != s').
+_CB_GEOM = dict(ra=1.02, rb=1.10, sigma_d=0.2)
+_CB_DRAWS = 4000000
+
+
+@pytest.mark.parametrize("n_trial", [1, 4, 10])
+def test_cb_two_sphere_fixed_move_ratio(n_trial):
+    """R-G1 / R-G2 / R-G3 pin.  CB samples the same AO weight as the plain rule: acc(r->r')/acc(r'->r) =
+    exp(n_R [V_ov(r') - V_ov(r)]), 4e6 draws per direction, tolerance 3 sigma + 1 % (the adopted form
+    leaves < 1 %, the printed prime-less Eq. 16 is 2-14 % off).  test_cb_ratio_pin_rejects_wrong_readings shows that
+    this very measurement fails for the printed form, for swapped forward/reverse roles and for a skipped 0/0 rule."""
+    n_R = workloads.config("C1").n_R()
+    err, sig, fwd, rev = _ratio_error(oracle.lib(), nd=_CB_DRAWS, n_trial=n_trial, n_R=n_R, **_CB_GEOM)
+    assert abs(err) < 3.0 * sig + 0.01, (n_trial, err, sig, fwd, rev)
+
+
+def _mutant_library(tmp_path, name, old, new):
+    """The oracle source with ONE textual substitution, compiled to a throw-away shared object (never the library the
+    parity tests use)."""
+    import ctypes as C
+    import subprocess
+    src = open(os.path.join(os.path.dirname(oracle.__file__), "hpmc_oracle.cpp")).read()
+    assert src.count(old) == 1, (name, src.count(old))
+    cpp, so = str(tmp_path / ("m_%s.cpp" % name)), str(tmp_path / ("m_%s.so" % name))
+    with open(cpp, "w") as f:
+        f.write(src.replace(old, new))
+    subprocess.run(["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC",
+                    "-o", so, cpp], check=True)
+    L_ = C.CDLL(so)
+    L_.oracle_create.restype = C.c_void_p
+    L_.oracle_create.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+    L_.oracle_build_cells.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32]
+    L_.oracle_eval_moves.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p,
+                                     C.c_double, C.c_int32, C.c_void_p]
+    L_.oracle_destroy.argtypes = [C.c_void_p]
+    L_.oracle_set_threads.argtypes = [C.c_int32]
+    return L_
+
+
+_EQ16 = "const float wk = (float)(Npins * (Npi + 1u)) / (float)((Nins + 1u) * Ni);"
+_MUTANTS = {
+    # the formula as PAPER.md L172 prints it: (N_i + 1) where the adopted reading R-G1 has (N'_i + 1)
+    "printed_eq16": (_EQ16, "const float wk = (float)(Npins * (Ni + 1u)) / (float)((Nins + 1u) * Ni);", (4, 10)),
+    # R-G2 with the roles of the forward (old centre) and reverse (new centre) counts exchanged
+    "roles_swapped": (_EQ16, "const float wk = (float)(Nins * (Ni + 1u)) / (float)((Npins + 1u) * Npi);", (4, 10)),
+    # R-G3 dropped: a rejecting depletant without a valid forward reinsertion is skipped instead of rejecting
+    "zero_rule_skipped": ("if (Npins == 0) return OUT_CB;", "if (Npins == 0) continue;", (1, 4)),
+}
+
+
+@pytest.mark.parametrize("name", sorted(_MUTANTS))
+def test_cb_ratio_pin_rejects_wrong_readings(tmp_path, name):
+    """The pin's resolving power, shown on throw-away builds of the oracle with ONE reading changed: each must FAIL
+    the tolerance of test_cb_two_sphere_fixed_move_ratio by at least half again (measured: printed form +3 % at n_trial = 4,
+    +16 % at 10; swapped roles +11 % / +56 %; skipped 0/0 rule > +100 %), while the adopted form sits at |err| < 0.3 %."""
+    old, new, trials = _MUTANTS[name]
+    L_ = _mutant_library(tmp_path, name, old, new)
+    n_R = workloads.config("C1").n_R()
+    for n_trial in trials:
+        err, sig, fwd, rev = _ratio_error(L_, nd=_CB_DRAWS, n_trial=n_trial, n_R=n_R, **_CB_GEOM)
+        assert abs(err) > 1.5 * (3.0 * sig + 0.01), (name, n_trial, err, sig, fwd, rev)
+
+
+def test_cb_zero_forward_weight_rule_thin_crescent():
+    """R-G3 on its own: a short step (d = 0.01, crescents 1.2 % of the insertion sphere) with n_trial = 1 makes
+    N'_ins = 0 the common case, so nearly every move with a rejecting depletant ends in outcome 5 through the 0/0
+    rule alone -- CB accepts only slightly more often than the plain rule -- and the forward/reverse ratio still
+    obeys detailed balance (it would not if the rule were anything but 'reject': see the mutant above)."""
+    n_R = workloads.config("C1").n_R()
+    g = dict(ra=1.05, rb=1.06, sigma_d=0.2)
+    nd = 2000000
+    L_ = oracle.lib()
+    err, sig, fwd, rev = _ratio_error(L_, nd=nd, n_trial=1, n_R=n_R, **g)
+    assert abs(err) < 3.0 * sig + 0.005, (err, sig)
+    pf, pr = _pair_counts(L_, g["ra"], g["rb"], nd, 0, n_R, g["sigma_d"])
+    # plain acceptance = P(no rejecting depletant); CB adds the moves whose (few) rejecting depletants all found a
+    # valid free reinsertion in ONE try: at most a few per cent of the rejected ones
+    for cb, plain in ((fwd, pf), (rev, pr)):
+        assert plain < cb < plain + 0.06 * (nd - plain), (cb, plain)
+    R = 0.6
+    assert abs((pf / pr) / math.exp(n_R * (lens(R, g["rb"]) - lens(R, g["ra"]))) - 1) < 3.0 * math.sqrt(1 / pf + 1 / pr)
 
 
 def test_cb_zero_trials_equals_plain_and_zero_density_is_hard_mc():
