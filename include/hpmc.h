@@ -44,15 +44,18 @@ typedef enum {
   HPMC_E_STATE = -3,             /* hpmc_sweep without hpmc_build_cells for the same (seed, step) */
   HPMC_E_DMAX = -4,              /* d_max > d_max_cap given at init */
   HPMC_E_CUDA = -5,              /* CUDA runtime error (message in hpmc_last_error) */
-  HPMC_E_NEIGHBOR_OVERFLOW = -6  /* more neighbours in range than the staging buffer holds (reported by the
-                                    next synchronising call; poses of that sweep are then invalid) */
+  HPMC_E_NEIGHBOR_OVERFLOW = -6  /* ONE move has more neighbours inside the list radius than the staging buffer holds
+                                    (reported and cleared by the next synchronising call; poses of that sweep are
+                                    then invalid).  Locally dense tiles do not raise it: the move kernel halves a
+                                    tile whose neighbour pool overflows and redoes it; the pool holds >= 768
+                                    neighbours, far more than hard particles can place around one move. */
 } hpmc_status;
 
 typedef struct {
   int32_t shape;       /* hpmc_shape */
   float sigma_c;       /* circumsphere diameter d_colloid: sphere diameter, 2 R_halfball, 2 (disk_a + disk_s) */
-  float disk_a;        /* spherodisk only */
-  float disk_s;        /* spherodisk only */
+  float disk_a;        /* spherodisk only: disk radius a >= 0 */
+  float disk_s;        /* spherodisk only: rounding radius s >= 0; sigma_c must equal 2 (a + s), else HPMC_E_BADARG */
   float sigma_d;       /* depletant diameter d_depletant (>= 0) */
   float box_L;         /* edge of the cubic periodic box */
   float d_max_cap;     /* largest d_max any later sweep will use; fixes the cell width

@@ -12,6 +12,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <algorithm>
 #include <string>
 #include <vector>
 
@@ -37,7 +38,17 @@ struct PoissonTable {
   size_t cap = 0;
 };
 
-struct EventPair { cudaEvent_t a, b; };
+struct QPlan {                         // how the item-queue move kernel is tiled over the active cells (moveq.cuh)
+  int ctas = 0;                        // CTAs, all resident at once
+  float ramp = 0.0f;                   // work ramp over the CTAs (one launch per pass only)
+  int cpc = 0, big = 0;                // average active cells per CTA, tile size
+  uint32_t* d_cta_first = nullptr;     // [ctas + 1] first active-cell index of every CTA's share
+  uint32_t* d_done = nullptr;          // [ctas] pass counters of the one-launch-per-sweep kernel
+  uint32_t seq = 0;                    // value of d_done[] before the next sweep
+  bool one_launch = false;             // all 8 passes in one cooperative launch (HPMC_SWEEP_LAUNCHES=8: one launch per pass)
+};
+
+struct EventPair { cudaEvent_t a, b; int n = 8; };
 
 }  // namespace
 
@@ -65,10 +76,9 @@ struct hpmc_ctx {
   size_t table_rr = 0;
   int num_sms = 148;
   int move_ctas = 0;
-  int q_ctas = 0;                      // CTAs of the item-queue move kernel
-  float q_ramp = 0.0f;                 // work ramp over the CTAs of the move kernel (see moveq.cuh)
-  int q_cpc = 0, q_big = 0;            // average active cells per CTA (one wave), tile size
+  QPlan plan[2];                       // launch plans of the item-queue move kernel: [0] plain rule, [1] configurational bias
   bool use_queue = true;               // HPMC_MOVE_KERNEL=warp selects the first (warp-per-cell) design
+  bool cb_queue = false;               // HPMC_CB_KERNEL=queue: configurational bias through the item-queue kernel too
   int64_t launches = 0;
   bool timing = false;
   std::vector<EventPair> ev;
@@ -192,13 +202,15 @@ int get_table(hpmc_ctx* ctx, double lambda, PoissonTable** out) {
 constexpr int QT = HPMC_QT;                // threads per CTA of the item-queue kernel
 template <int SHAPE> struct QCfg { static constexpr int CPT = SHAPE == SH_SPHERE ? HPMC_QCPT : 1; };   // tile capacity CPT*QT cells
 
-template <int SHAPE>
+template <int SHAPE, bool CB>
 int setup_moveq(hpmc_ctx* ctx) {
-  const size_t smem = QSmem<SHAPE, QT, QCfg<SHAPE>::CPT>::bytes;
-  cudaError_t e = cudaFuncSetAttribute(k_moveq<SHAPE, QT, QCfg<SHAPE>::CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  QPlan& P = ctx->plan[CB ? 1 : 0];
+  using SM = QSmem<SHAPE, QT, QCfg<SHAPE>::CPT, CB>;
+  const size_t smem = SM::bytes;
+  cudaError_t e = cudaFuncSetAttribute(k_moveq<SHAPE, QT, QCfg<SHAPE>::CPT, CB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return fail(ctx, HPMC_E_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
   int per_sm = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_moveq<SHAPE, QT, QCfg<SHAPE>::CPT>, QT, smem);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_moveq<SHAPE, QT, QCfg<SHAPE>::CPT, CB>, QT, smem);
   if (e != cudaSuccess || per_sm < 1) return fail(ctx, HPMC_E_CUDA, "k_moveq does not fit on an SM");
   // one wave: every CTA of a pass is resident at once (a pass is latency-, not throughput-bound) and owns
   // cells_per_cta active cells, worked through in nsub tiles of equal size
@@ -207,15 +219,17 @@ int setup_moveq(hpmc_ctx* ctx) {
   int cpc = (nact + resident - 1) / resident;
   int pool_cap = 1 << 30;
   {
-    // keep the expected number of listed neighbours of a tile within the shared-memory pool (the error flag
-    // HPMC_E_NEIGHBOR_OVERFLOW stays as the backstop): ideal-gas estimate of the neighbours inside the list radius,
-    // times 2 (contact shell of a dense hard-particle fluid or crystal), for every non-empty cell of the tile
+    // keep the expected number of listed neighbours of a tile within the shared-memory pool: ideal-gas estimate of
+    // the neighbours inside the list radius from the MEAN density, times 2 (contact shell of a dense hard-particle
+    // fluid or crystal), for every non-empty cell of the tile.  Only a performance heuristic: a tile that overflows
+    // anyway (a cluster in a dilute box) is halved and redone inside the kernel
     const double L = ctx->p.box_L, dens = (double)ctx->N / (L * L * L);
-    const double rl = (double)ctx->p.sigma_c + ctx->p.sigma_d + 1e-3;
+    const double rl = CB ? std::sqrt((double)ctx->g.rcut2) : (double)ctx->p.sigma_c + ctx->p.sigma_d + 1e-3;
     const double nbr = 2.0 * dens * (4.0 * M_PI / 3.0) * rl * rl * rl + 1.0;
     const double occ = (double)ctx->N / (double)ctx->ncell;
     const double pmove = occ < 1.0 ? occ : 1.0;
-    pool_cap = (int)((double)QSmem<SHAPE, QT, QCfg<SHAPE>::CPT>::POOL / (nbr * pmove));
+    pool_cap = (int)((double)SM::POOL / (nbr * pmove));
+    if (getenv("HPMC_POOL_CAP_OFF")) pool_cap = 1 << 30;      // tests: rely on the in-kernel tile splitting alone
     if (cpc > pool_cap) cpc = pool_cap;
   }
   if (cpc < 8) cpc = 8;   // small systems are latency-bound: more, smaller CTAs (measured on C1, C2, C4)
@@ -223,7 +237,16 @@ int setup_moveq(hpmc_ctx* ctx) {
   constexpr int QM = QCfg<SHAPE>::CPT * QT;
   // work ramp: only when the pass is one full wave (then every SM holds per_sm CTAs launched in index order)
   float ramp = 0.0f;
-  if ((nact + cpc - 1) / cpc > resident / 2) {
+  {
+    int dev = 0, coop = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+    const char* sl = getenv("HPMC_SWEEP_LAUNCHES");
+    P.one_launch = coop != 0 && !(sl && atoi(sl) == 8);
+  }
+  // (the ramp only pays when all CTAs start a pass together, i.e. with one launch per pass: measured at C3 in the
+  // one-launch kernel 0.2 / 0.1 / 0 -> 505 / 482 / 475 us per sweep)
+  if (!P.one_launch && (nact + cpc - 1) / cpc > resident / 2) {
     ramp = 0.2f;    // measured at C3: 0 / 0.1 / 0.15 / 0.2 -> 66.7 / 65.3 / 64.2 / 63.7 us per pass
     if (const char* o = getenv("HPMC_RAMP")) ramp = (float)atof(o);
     if (ramp < 0.0f) ramp = 0.0f;
@@ -231,35 +254,67 @@ int setup_moveq(hpmc_ctx* ctx) {
   }
   if ((double)cpc * (1.0 + ramp) > (double)pool_cap) cpc = (int)((double)pool_cap / (1.0 + ramp));
   if (cpc < 8) cpc = 8;
-  ctx->q_ramp = ramp;
+  P.ramp = ramp;
   const int cmax = (int)std::ceil((double)cpc * (1.0 + ramp)) + 1;     // largest share of a CTA
   int nsub = (cmax + QM - 1) / QM;
   int big = (cmax + nsub - 1) / nsub;
   if (big > QM) big = QM;
   if (const char* o = getenv("HPMC_TILE_BIG")) { const int v = atoi(o); if (v >= 1 && v <= QM) big = v; }
-  ctx->q_cpc = cpc; ctx->q_big = big;
-  ctx->q_ctas = (nact + cpc - 1) / cpc;
+  P.cpc = cpc; P.big = big;
+  P.ctas = (nact + cpc - 1) / cpc;
+  {
+    // shares: CTA i owns [first(i), first(i+1)), first(i) = nact (x + ramp x (1 - x)), x = i / n: the first CTAs get
+    // (1 + ramp) times the average share, the last ones (1 - ramp) times
+    const int n = P.ctas;
+    std::vector<uint32_t> first((size_t)n + 1);
+    for (int i = 0; i <= n; ++i) {
+      const double x = (double)i / (double)n;
+      const double v = (double)nact * (x + (double)ramp * x * (1.0 - x));
+      first[(size_t)i] = i >= n ? (uint32_t)nact : std::min((uint32_t)v, (uint32_t)nact);
+    }
+    cudaError_t e2 = cudaMalloc(&P.d_cta_first, sizeof(uint32_t) * ((size_t)n + 1));
+    if (e2 == cudaSuccess) e2 = cudaMalloc(&P.d_done, sizeof(uint32_t) * (size_t)n);
+    if (e2 == cudaSuccess) e2 = cudaMemcpy(P.d_cta_first, first.data(), sizeof(uint32_t) * ((size_t)n + 1), cudaMemcpyHostToDevice);
+    if (e2 == cudaSuccess) e2 = cudaMemset(P.d_done, 0, sizeof(uint32_t) * (size_t)n);
+    if (e2 != cudaSuccess) return fail(ctx, HPMC_E_CUDA, std::string("setup_moveq: ") + cudaGetErrorString(e2));
+    // every CTA of the one-launch kernel must be resident at once (its CTAs wait for one another)
+    P.one_launch = P.one_launch && n <= resident && n <= 32 * SM::NBMAP_WORDS;
+  }
   if (getenv("HPMC_VERBOSE"))
-    fprintf(stderr, "k_moveq<%d,%d>: smem %zu B, %d CTAs/SM, %d CTAs x %d cells on average (ramp %.2f), tiles of %d\n", SHAPE,
-            QT, smem, per_sm, ctx->q_ctas, cpc, (double)ramp, big);
+    fprintf(stderr, "k_moveq<%d,%d,%s>: smem %zu B, %d CTAs/SM, %d CTAs x %d cells on average (ramp %.2f), tiles of %d, %s\n", SHAPE,
+            QT, CB ? "cb" : "plain", smem, per_sm, P.ctas, cpc, (double)ramp, big, P.one_launch ? "one launch per sweep" : "one launch per pass");
   return 0;
 }
 
-template <int SHAPE>
-int launch_moveq(hpmc_ctx* ctx, const MoveArgs& a, const PoissonTable* pt) {
+template <int SHAPE, bool CB>
+int launch_moveq(hpmc_ctx* ctx, const MoveArgs& a, const PoissonTable* pt, const uint32_t* perm8) {
+  QPlan& P = ctx->plan[CB ? 1 : 0];
+  using SM = QSmem<SHAPE, QT, QCfg<SHAPE>::CPT, CB>;
   QArgs q;
   q.m = a;
+  q.cta_first = P.d_cta_first; q.done = P.d_done; q.seq0 = P.seq;
+  q.npass = perm8 ? 8 : 1;
+  for (int i = 0; i < 8; ++i) q.colours[i] = perm8 ? perm8[i] : 0u;
   q.magic_hc = ~0ull / (unsigned long long)a.hc + 1ull;   // floor((2^64-1)/hc)+1 == floor(2^64/hc)+1 unless hc | 2^64
   if ((a.hc & (a.hc - 1)) == 0) q.magic_hc = (1ull << 63) / (unsigned long long)a.hc * 2ull + 1ull;
   q.pguide = pt->has_guide ? pt->d_G : nullptr;
-  q.ramp = ctx->q_ramp; q.tile_cells = ctx->q_big;
+  q.ramp = P.ramp; q.tile_cells = P.big;
   q.wlo = 2.1f * a.g.w; q.whi = a.g.L - 2.1f * a.g.w;
   {
     const float rl = (ctx->p.sigma_c + ctx->p.sigma_d) + 1e-3f;
     q.rlist2 = rl * rl;
-    if (q.rlist2 > a.g.rcut2) q.rlist2 = a.g.rcut2;
+    if (CB || q.rlist2 > a.g.rcut2) q.rlist2 = a.g.rcut2;      // CB also samples about the OLD centre: the full r_cut of R-3.4
   }
-  k_moveq<SHAPE, QT, QCfg<SHAPE>::CPT><<<ctx->q_ctas, QT, QSmem<SHAPE, QT, QCfg<SHAPE>::CPT>::bytes, ctx->stream>>>(q);
+  if (perm8) {
+    // cooperative launch: the runtime guarantees that all CTAs are resident, which the neighbour waits rely on
+    void* args[] = {(void*)&q};
+    const cudaError_t e = cudaLaunchCooperativeKernel((const void*)k_moveq<SHAPE, QT, QCfg<SHAPE>::CPT, CB>, dim3(P.ctas),
+                                                      dim3(QT), args, SM::bytes, ctx->stream);
+    if (e != cudaSuccess) return fail(ctx, HPMC_E_CUDA, std::string("cudaLaunchCooperativeKernel: ") + cudaGetErrorString(e));
+    P.seq += 8u;
+    return 0;
+  }
+  k_moveq<SHAPE, QT, QCfg<SHAPE>::CPT, CB><<<P.ctas, QT, SM::bytes, ctx->stream>>>(q);
   return 0;
 }
 
@@ -283,6 +338,12 @@ int hpmc_init(hpmc_ctx** out, const hpmc_params* p, int64_t N, float* d_pos4, fl
   if (!(p->box_L > 0.0f) || !(p->sigma_c > 0.0f) || p->sigma_d < 0.0f || p->d_max_cap < 0.0f)
     return fail(nullptr, HPMC_E_BADARG, "hpmc_init: bad geometry parameters");
   if (p->shape < HPMC_SPHERE || p->shape > HPMC_SPHERODISK) return fail(nullptr, HPMC_E_BADARG, "hpmc_init: bad shape");
+  if (p->shape == HPMC_SPHERODISK) {
+    // sigma_c is the circumsphere diameter 2 (a + s): the insertion radius, the cell width and the list radius derive from it
+    if (!(p->disk_a >= 0.0f) || !(p->disk_s >= 0.0f) || !(p->disk_a + p->disk_s > 0.0f) ||
+        std::fabs((double)p->sigma_c - 2.0 * ((double)p->disk_a + (double)p->disk_s)) > 1e-5 * (double)p->sigma_c)
+      return fail(nullptr, HPMC_E_BADARG, "hpmc_init: spherodisk needs disk_a, disk_s >= 0 and sigma_c == 2 (disk_a + disk_s)");
+  }
   if (p->shape != HPMC_SPHERE && d_pos4 && !d_quat4)
     return fail(nullptr, HPMC_E_BADARG, "hpmc_init: anisotropic shape needs orientations");
   if (!d_pos4 && d_quat4) return fail(nullptr, HPMC_E_BADARG, "hpmc_init: d_quat4 without d_pos4");
@@ -337,11 +398,16 @@ int hpmc_init(hpmc_ctx** out, const hpmc_params* p, int64_t N, float* d_pos4, fl
   {
     const char* sel = getenv("HPMC_MOVE_KERNEL");
     ctx->use_queue = !(sel && std::string(sel) == "warp");
+    // Configurational bias runs on the warp-per-cell kernel by default: measured on spherodisks with n_trial = 4 it is
+    // 1.2-1.75x faster than the round-based CB stage of the item-queue kernel at every size tried (32,768 ... 884,736
+    // particles; profiles/r2_cb_kernels.md).  Both are bit-exact against the oracle and both are tested.
+    const char* cbk = getenv("HPMC_CB_KERNEL");
+    ctx->cb_queue = cbk && std::string(cbk) == "queue";
     int rc = 0;
     switch (p->shape) {
-      case HPMC_SPHERE: rc = setup_moveq<SH_SPHERE>(ctx); break;
-      case HPMC_HALFBALL: rc = setup_moveq<SH_HALFBALL>(ctx); break;
-      default: rc = setup_moveq<SH_SPHERODISK>(ctx); break;
+      case HPMC_SPHERE: rc = setup_moveq<SH_SPHERE, false>(ctx); if (!rc) rc = setup_moveq<SH_SPHERE, true>(ctx); break;
+      case HPMC_HALFBALL: rc = setup_moveq<SH_HALFBALL, false>(ctx); if (!rc) rc = setup_moveq<SH_HALFBALL, true>(ctx); break;
+      default: rc = setup_moveq<SH_SPHERODISK, false>(ctx); if (!rc) rc = setup_moveq<SH_SPHERODISK, true>(ctx); break;
     }
     if (rc) { g_init_error = ctx->err; hpmc_destroy(ctx); return rc; }
   }
@@ -356,6 +422,7 @@ void hpmc_destroy(hpmc_ctx* ctx) {
   cudaFree(ctx->d_cpos); cudaFree(ctx->d_caxis); cudaFree(ctx->d_cid); cudaFree(ctx->d_rank);
   cudaFree(ctx->d_cell_pid); cudaFree(ctx->d_counts); cudaFree(ctx->d_cell_start); cudaFree(ctx->d_tile_sums);
   cudaFree(ctx->d_outcome); cudaFree(ctx->d_counters); cudaFree(ctx->d_err);
+  for (auto& pl : ctx->plan) { cudaFree(pl.d_cta_first); cudaFree(pl.d_done); }
   for (auto& t : ctx->tables) { cudaFree(t.d_T); cudaFree(t.d_G); }
   for (auto& e : ctx->ev) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
   delete ctx;
@@ -441,15 +508,27 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
     ep = &ctx->ev[ctx->ev_used++];
     CU(cudaEventRecord(ep->a, ctx->stream));
   }
-  for (int pass = 0; pass < 8; ++pass) {
-    a.colour = perm[pass];
-    if (ctx->use_queue && !cb) {
+  int nlaunch = 8;
+  if (ctx->use_queue && (!cb || ctx->cb_queue)) {
+    // item-queue kernel (moveq.cuh): one cooperative launch for the 8 passes (CTAs synchronise with their spatial
+    // neighbours only), or one launch per pass
+    const bool one = ctx->plan[cb ? 1 : 0].one_launch;
+    for (int pass = 0; pass < (one ? 1 : 8); ++pass) {
+      a.colour = perm[pass];
+      const uint32_t* p8 = one ? perm : nullptr;
+      int rc2 = 0;
       switch (ctx->p.shape) {
-        case HPMC_SPHERE: launch_moveq<SH_SPHERE>(ctx, a, pt); break;
-        case HPMC_HALFBALL: launch_moveq<SH_HALFBALL>(ctx, a, pt); break;
-        default: launch_moveq<SH_SPHERODISK>(ctx, a, pt); break;
+        case HPMC_SPHERE: rc2 = cb ? launch_moveq<SH_SPHERE, true>(ctx, a, pt, p8) : launch_moveq<SH_SPHERE, false>(ctx, a, pt, p8); break;
+        case HPMC_HALFBALL: rc2 = cb ? launch_moveq<SH_HALFBALL, true>(ctx, a, pt, p8) : launch_moveq<SH_HALFBALL, false>(ctx, a, pt, p8); break;
+        default: rc2 = cb ? launch_moveq<SH_SPHERODISK, true>(ctx, a, pt, p8) : launch_moveq<SH_SPHERODISK, false>(ctx, a, pt, p8); break;
       }
-    } else {
+      if (rc2) return rc2;
+    }
+    if (one) nlaunch = 1;
+  } else {
+    // first design (move.cuh, HPMC_MOVE_KERNEL=warp): one warp per active cell, one launch per pass
+    for (int pass = 0; pass < 8; ++pass) {
+      a.colour = perm[pass];
       switch (ctx->p.shape) {
         case HPMC_SPHERE: launch_move<SH_SPHERE>(ctx, a, cb); break;
         case HPMC_HALFBALL: launch_move<SH_HALFBALL>(ctx, a, cb); break;
@@ -457,8 +536,8 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
       }
     }
   }
-  if (ep) CU(cudaEventRecord(ep->b, ctx->stream));
-  ctx->launches += 8;
+  if (ep) { CU(cudaEventRecord(ep->b, ctx->stream)); ep->n = nlaunch; }
+  ctx->launches += nlaunch;
   CU(cudaGetLastError());
   ctx->built = false;
   return HPMC_OK;
@@ -479,7 +558,15 @@ static int check_err_flag(hpmc_ctx* ctx) {
   int e = 0;
   CU(cudaMemcpyAsync(&e, ctx->d_err, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
-  if (e) return fail(ctx, HPMC_E_NEIGHBOR_OVERFLOW, "move kernel: more than MAXNB neighbours in range");
+  if (e == 2) {
+    CU(cudaMemsetAsync(ctx->d_err, 0, sizeof(int), ctx->stream));
+    return fail(ctx, HPMC_E_CUDA, "move kernel: a CTA waited too long for a neighbouring CTA's pass (poses of that sweep are invalid)");
+  }
+  if (e) {
+    CU(cudaMemsetAsync(ctx->d_err, 0, sizeof(int), ctx->stream));
+    return fail(ctx, HPMC_E_NEIGHBOR_OVERFLOW, "move kernel: one move has more neighbours inside the list radius than the "
+                                               "shared-memory pool (item-queue kernel) or MAXNB = 64 (warp kernel) holds");
+  }
   return HPMC_OK;
 }
 
@@ -568,7 +655,7 @@ int hpmc_move_kernel_ms(hpmc_ctx* ctx, double* ms_total, int64_t* launches) {
     CU(cudaEventElapsedTime(&ms, ctx->ev[i].a, ctx->ev[i].b));
     ctx->ev_ms += ms;
   }
-  ctx->ev_launches += 8 * (int64_t)ctx->ev_used;
+  for (size_t i = 0; i < ctx->ev_used; ++i) ctx->ev_launches += ctx->ev[i].n;
   ctx->ev_used = 0;
   *ms_total = ctx->ev_ms; *launches = ctx->ev_launches;
   return HPMC_OK;

@@ -47,6 +47,14 @@ struct QArgs {
   float wlo, whi;                  // 2.1 w and L - 2.1 w: centres in between need no minimum image (phase 1b)
   float ramp;                      // share of the first / last CTA relative to the average: 1 + ramp / 1 - ramp
   int tile_cells;                  // a CTA works through its share in tiles of tile_cells <= CPT*T cells (normally one)
+  // ---- one launch per sweep (npass = 8): a CTA keeps its share of the active-cell index space for all 8 colours
+  // and runs the passes back to back.  Instead of a grid-wide barrier it waits, before the neighbourhood walk of pass
+  // p, only for the CTAs whose shares touch its own 27-cell neighbourhoods to have published pass p-1 (done[b] >= seq0 + p).
+  int npass;                       // 1: the colour in m.colour (one launch per pass); 8: colours[0..7] in this launch
+  uint32_t colours[8];
+  const uint32_t* cta_first;       // [gridDim.x + 1] first active-cell index of every CTA's share (host table, with the ramp)
+  uint32_t* done;                  // [gridDim.x] passes published so far (monotone over the sweeps of a context)
+  uint32_t seq0;                   // value of done[] before this sweep
   float rlist2;                    // neighbours farther than this from the new centre cannot touch any depletant
                                    // of the move: (sigma_c + sigma_d + 1e-3)^2 for the plain rule (insertion
                                    // sphere about the new centre only), r_cut^2 of R-3.4 otherwise
@@ -76,7 +84,11 @@ struct QLayout {
 };
 
 // shared-memory carve-up for a CTA of T threads handling tiles of up to M = CPT*T active cells (hence <= M moves)
-template <int SHAPE, int T, int CPT>
+#ifndef HPMC_CB_WINDOW
+#define HPMC_CB_WINDOW 32          // configurational bias: depletant indices examined per round and move (speculation bound)
+#endif
+
+template <int SHAPE, int T, int CPT, bool CB = false>
 struct QSmem {
   using Lq = QLayout<SHAPE>;
   static constexpr int M = CPT * T;
@@ -100,7 +112,20 @@ struct QSmem {
   static constexpr size_t o_alive = o_scal + 32;                                // u16[M]
   static constexpr size_t o_ovf = o_alive + 2 * M;                              // u32[T] overflow queue of phase 1b
   static constexpr size_t o_cnt = o_ovf + 4 * T;                                // u32[16] CTA totals of the counters
-  static constexpr size_t bytes = o_cnt + 64;
+  static constexpr size_t o_tcnt = o_cnt + 64;                                  // u32[4] phase-1a counters of the tile in flight
+  static constexpr int NBMAP_WORDS = T <= 64 ? 160 : 40;                                        // bitmap over <= 1280 CTAs (8 per SM on 148 SMs fit; the 28,160 B that allow 8 CTAs per SM leave no more room)
+  static constexpr size_t o_nbmap = o_tcnt + 16;                                // u32[NBMAP_WORDS] CTAs this one must wait for
+  // configurational bias (a9): per move the product so far, the rejecting depletants handled, the window start, the
+  // head of its job list; per job (one rejecting depletant of the current window) k, move | next, packed counts
+  static constexpr int JCAP = CB ? 4 * T : 0;
+  static constexpr size_t o_P = o_nbmap + 4 * NBMAP_WORDS;                       // float[M]
+  static constexpr size_t o_cbre = o_P + (CB ? 4 * M : 0);                       // u32[M] jobs counted (x 2 n_trial = reinsertions)
+  static constexpr size_t o_klo = o_cbre + (CB ? 4 * M : 0);                     // u32[M]
+  static constexpr size_t o_jhead = o_klo + (CB ? 4 * M : 0);                    // int[M]
+  static constexpr size_t o_jk = o_jhead + (CB ? 4 * M : 0);                     // u32[JCAP]
+  static constexpr size_t o_jm = o_jk + 4 * JCAP;                                // u32[JCAP] move | (next job + 1) << 16
+  static constexpr size_t o_jc = o_jm + 4 * JCAP;                                // uint2[JCAP] (N_i | N'_ins << 16, N'_i | N_ins << 16)
+  static constexpr size_t bytes = o_jc + 8 * JCAP;
 };
 
 template <int SHAPE>
@@ -141,16 +166,22 @@ __device__ __forceinline__ uint32_t poisson_count(const unsigned long long* __re
   return (uint32_t)lo;
 }
 
-// Pointers to the phase-2 tables of one CTA: its own shared memory, or (thread-block clusters) a peer's through
-// distributed shared memory.
+// Pointers to the phase-2 tables of one CTA.
 struct QTables {
   const float4* r1; const float4* rho; const float4* aold; const float4* anew; const float4* pool;
-  const uint32_t* Nd; uint32_t* knext; uint32_t* rejmin; const int* head; uint32_t* todo; const uint16_t* alive;
+  uint32_t* knext; uint32_t* rejmin; const int* head; uint32_t* todo; const uint16_t* alive;
+  // configurational bias: job list of the current window
+  uint32_t* jk; uint32_t* jm; uint2* jc; int* jhead; uint32_t* njobs; int jcap;
 };
 
+#ifndef HPMC_LANES_PER_OPEN_MOVE
+#define HPMC_LANES_PER_OPEN_MOVE 0      // > 0: a lane looking for work retires once t >= this x (open moves): fewer helpers at the end of a tile
+#endif
+
 // Phase 2 (a8): the depletant item queue over the `nalive` surviving moves described by `tb`; returns when no move
-// of the tile has unclaimed work left and this thread's last item is done.
-template <int SHAPE>
+// of the tile has unclaimed work left and this thread's last item is done.  rejmin[m] starts at N_d and only
+// decreases, so "k < rejmin[m]" is the one test for "this depletant still matters".
+template <int SHAPE, bool CB>
 __device__ __forceinline__ void q_depletant_queue(const QTables& tb, int nalive, const Geo& g, const Key10& key,
                                                   uint32_t c3dep, int t, uint32_t& n_eval, uint32_t& n_blocks) {
   constexpr bool ANISO = SHAPE != SH_SPHERE;
@@ -158,7 +189,7 @@ __device__ __forceinline__ void q_depletant_queue(const QTables& tb, int nalive,
   const int nw_alive = (nalive + 31) >> 5;
   int j = t % nalive;
   uint32_t m = tb.alive[j];
-  uint32_t c_pid = __float_as_uint(tb.r1[m].w), c_Nd = tb.Nd[m];
+  uint32_t c_pid = __float_as_uint(tb.r1[m].w);
   int c_head = tb.head[m];
   float4 c_rho = tb.rho[m];
   V3 c_aold = V3{0.f, 0.f, 1.f}, c_anew = V3{0.f, 0.f, 1.f};
@@ -168,7 +199,7 @@ __device__ __forceinline__ void q_depletant_queue(const QTables& tb, int nalive,
   }
   volatile uint32_t* v_rejmin = tb.rejmin;
   volatile uint32_t* v_todo = tb.todo;
-  uint32_t k = 0, att = 0, trip = 0;
+  uint32_t k = 0, c3 = c3dep, trip = 0;
   bool have = false, active = true;
   for (;;) {
     // ---- claim (divergent, short): lanes without an item take the next k of their move, or re-attach
@@ -176,26 +207,29 @@ __device__ __forceinline__ void q_depletant_queue(const QTables& tb, int nalive,
 #pragma unroll 1
       for (;;) {
         k = atomicAdd(&tb.knext[m], 1u);
-        if (k < min(c_Nd, v_rejmin[m])) { att = 0; have = true; break; }
-        // this move has no unclaimed work left: retire its bit, attach to an unfinished move of the tile
+        if (k < v_rejmin[m]) { c3 = c3dep; have = true; break; }
+        // this move has no unclaimed work left: retire its bit (idempotent), attach to an unfinished move of the tile
         atomicAnd(&tb.todo[j >> 5], ~(1u << (j & 31)));
         int found = -1;
         int wi = j >> 5;
+        uint32_t open = 0;
 #pragma unroll 1
         for (int i = 0; i < nw_alive; ++i) {            // only the words that ever held a bit
           const uint32_t w = v_todo[wi];
-          if (w) {
+          if (HPMC_LANES_PER_OPEN_MOVE > 0) open += __popc(w);
+          if (w && found < 0) {
             const int r = t & 31;
             const uint32_t w2 = __funnelshift_r(w, w, r);
             found = wi * 32 + ((__ffs(w2) - 1 + r) & 31);
-            break;
+            if (HPMC_LANES_PER_OPEN_MOVE == 0) break;
           }
           wi = (wi + 1 == nw_alive) ? 0 : wi + 1;
         }
+        if (HPMC_LANES_PER_OPEN_MOVE > 0 && (uint32_t)t >= HPMC_LANES_PER_OPEN_MOVE * open) found = -1;
         if (found < 0) { active = false; break; }
         j = found;
         m = tb.alive[j];
-        c_pid = __float_as_uint(tb.r1[m].w); c_Nd = tb.Nd[m]; c_head = tb.head[m]; c_rho = tb.rho[m];
+        c_pid = __float_as_uint(tb.r1[m].w); c_head = tb.head[m]; c_rho = tb.rho[m];
         if (ANISO) {
           const float4 ao = tb.aold[m], an = tb.anew[m];
           c_aold = V3{ao.x, ao.y, ao.z}; c_anew = V3{an.x, an.y, an.z};
@@ -206,30 +240,46 @@ __device__ __forceinline__ void q_depletant_queue(const QTables& tb, int nalive,
     // (checked every fourth trip: a warp that has run dry idles through at most three cheap trips)
     if ((++trip & 3u) == 0u && !__any_sync(0xffffffffu, active)) break;
     if (active) {
-      // one Philox block = one cube-rejection attempt of depletant k (R-S3)
-      const Block4 r = philox(key, c_pid, k, 0, c3dep + (att << 16));
+      // one Philox block = one cube-rejection attempt of depletant k (R-S3); c3 carries the attempt number
+      const Block4 r = philox(key, c_pid, k, 0, c3);
       ++n_blocks;
       V3 d = V3{g.Rins * sym_unit_bits(r.x), g.Rins * sym_unit_bits(r.y), g.Rins * sym_unit_bits(r.z)};
-      bool inside = dot3(d, d) <= g.Rins2;
-      if (!inside && att == 63u) { d = V3{0.f, 0.f, 0.f}; inside = true; }
+      float d2 = dot3(d, d);
+      bool inside = d2 <= g.Rins2;
+      if (!inside && c3 >= c3dep + (63u << 16)) { d = V3{0.f, 0.f, 0.f}; d2 = 0.0f; inside = true; }
       if (inside) {
         ++n_eval;
         const V3 ro = V3{c_rho.x, c_rho.y, c_rho.z};
-        if (q_new_only<SHAPE>(g, d, ro, c_aold, c_anew) && q_free_of_nbrs<SHAPE>(g, tb.pool, c_head, d))
-          atomicMin(&tb.rejmin[m], k);
+        // new-only (L72): overlaps the new pose (|d|^2 < R^2 is dep_overlap's own first test, same value as d2) ...
+        bool hit;
+        if (ANISO) hit = q_new_only<SHAPE>(g, d, ro, c_aold, c_anew);
+        else { const V3 e = d - ro; hit = (d2 < g.Rins2) && !(dot3(e, e) < g.Rins2); }
+        if (hit && q_free_of_nbrs<SHAPE>(g, tb.pool, c_head, d)) {
+          if (!CB) {
+            atomicMin(&tb.rejmin[m], k);
+            atomicAnd(&tb.todo[j >> 5], ~(1u << (j & 31)));   // every k below this one is already claimed: closed for newcomers
+          } else {
+            // Sec. III.D: a rejecting depletant does not end the move; it becomes a reinsertion job of this window
+            const uint32_t jb = atomicAdd(tb.njobs, 1u);
+            if (jb < (uint32_t)tb.jcap) {
+              const int prev = atomicExch(&tb.jhead[m], (int)jb);
+              tb.jk[jb] = k; tb.jm[jb] = m | ((uint32_t)(prev + 1) << 16); tb.jc[jb] = make_uint2(0u, 0u);
+            }
+          }
+        }
         have = false;
       } else {
-        ++att;
+        c3 += 1u << 16;
         if (k > v_rejmin[m]) have = false;     // a lower k already rejects: this one cannot matter
       }
     }
   }
 }
 
-template <int SHAPE, int T, int CPT>
-__global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QArgs Q) {
+template <int SHAPE, int T, int CPT, bool CB>
+__global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS)) k_moveq(const QArgs Q) {
   using Lq = QLayout<SHAPE>;
-  using S = QSmem<SHAPE, T, CPT>;
+  using S = QSmem<SHAPE, T, CPT, CB>;
   constexpr bool ANISO = Lq::ANISO;
   constexpr int E = Lq::ENTRY;
   constexpr int M = S::M, POOL = S::POOL, HCAP = S::HCAP, NW = M / 32;
@@ -258,34 +308,72 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
   uint16_t* s_alive = reinterpret_cast<uint16_t*>(sb_ + S::o_alive);
   uint32_t* s_ovf = reinterpret_cast<uint32_t*>(sb_ + S::o_ovf);
   uint32_t* s_cnt = reinterpret_cast<uint32_t*>(sb_ + S::o_cnt);
+  uint32_t* s_tcnt = reinterpret_cast<uint32_t*>(sb_ + S::o_tcnt);  // [0] trials_trans [1] trials_rot [2] rej_boundary of this tile
+  float* s_P = reinterpret_cast<float*>(sb_ + S::o_P);               // configurational bias only (CB)
+  uint32_t* s_cbre = reinterpret_cast<uint32_t*>(sb_ + S::o_cbre);
+  uint32_t* s_klo = reinterpret_cast<uint32_t*>(sb_ + S::o_klo);
+  int* s_jhead = reinterpret_cast<int*>(sb_ + S::o_jhead);
+  uint32_t* s_jk = reinterpret_cast<uint32_t*>(sb_ + S::o_jk);
+  uint32_t* s_jm = reinterpret_cast<uint32_t*>(sb_ + S::o_jm);
+  uint2* s_jc = reinterpret_cast<uint2*>(sb_ + S::o_jc);
 
   const int t = threadIdx.x;
   const int nc = g.nc, hc = A.hc;
-  const int px = A.colour & 1, py = (A.colour >> 1) & 1, pz = (A.colour >> 2) & 1;
-  const uint32_t colw = A.colour << 8;
-  const uint32_t c3dep = P_DEPPOS + colw;
-
-  // per-thread counters (reduced once at the end of the kernel)
-  // counters: the two that tick in the hot loop live in registers; the per-move ones go straight to CTA totals in
-  // shared memory (CTA totals stay far below 2^32), so that they do not occupy registers across phase 2
+  // per-thread counters (reduced once at the end of the kernel): the two that tick in the hot loop live in
+  // registers; the per-move ones go to CTA totals in shared memory (far below 2^32)
   uint32_t n_eval = 0, n_blocks = 0;
   if (t < C_COUNT) s_cnt[t] = 0u;               // ordered before the first use by the barrier at the top of the tile loop
 
-  // CTA b owns the active cells [lo(b), lo(b+1)), lo(i) = nact (x + ramp x (1 - x)), x = i / gridDim.x: the first CTAs
-  // get (1 + ramp) times the average share, the last ones (1 - ramp) times.  The SM's warp arbitration favours the
-  // CTAs that were launched first; with equal shares the last-launched CTA of every SM ends the pass alone.
-  auto range_lo = [&](uint32_t i) -> uint32_t {
-    const double x = (double)i / (double)gridDim.x;
-    const double v = (double)A.nact * (x + (double)Q.ramp * x * (1.0 - x));
-    return i >= gridDim.x ? (uint32_t)A.nact : min((uint32_t)v, (uint32_t)A.nact);
-  };
-  const uint32_t cta_lo = range_lo(blockIdx.x);
-  const uint32_t cta_hi = range_lo(blockIdx.x + 1u);
+  // CTA b owns the active-cell indices [cta_first[b], cta_first[b+1]) for every colour; the host table gives the
+  // first-launched CTAs a larger share (the SM's warp arbitration favours them; see setup_moveq).
+  const uint32_t cta_lo = Q.cta_first[blockIdx.x];
+  const uint32_t cta_hi = Q.cta_first[blockIdx.x + 1u];
+
+  // ---- neighbour CTAs (npass > 1): every CTA whose share holds a cell of the x-rows (az+dz, ay+dy), dz, dy in
+  // {-1,0,1}, of the rows this share touches -- a superset of the 27-cell neighbourhoods of its cells.  Bitmap over CTAs.
+  uint32_t* s_nbmap = reinterpret_cast<uint32_t*>(sb_ + S::o_nbmap);
+  if (Q.npass > 1) {
+    for (int w = t; w < S::NBMAP_WORDS; w += T) s_nbmap[w] = 0u;
+    __syncthreads();
+    if (cta_hi > cta_lo) {
+      const int r_lo = (int)(cta_lo / (uint32_t)hc), r_hi = (int)((cta_hi - 1u) / (uint32_t)hc);
+      const int nrow = r_hi - r_lo + 1;
+      for (int it = t; it < nrow * 9; it += T) {
+        const int r = r_lo + it / 9, o = it % 9;
+        int az = r / hc + (o / 3 - 1), ay = r % hc + (o % 3 - 1);
+        az += (az < 0) ? hc : 0; az -= (az >= hc) ? hc : 0;
+        ay += (ay < 0) ? hc : 0; ay -= (ay >= hc) ? hc : 0;
+        const uint32_t a0 = (uint32_t)(az * hc + ay) * (uint32_t)hc, a1 = a0 + (uint32_t)hc - 1u;
+        // CTAs owning a0 and a1: largest b with cta_first[b] <= a
+        uint32_t b0 = 0, b1 = 0;
+        {
+          uint32_t lo = 0, hi = gridDim.x;
+          while (hi - lo > 1u) { const uint32_t mid = (lo + hi) >> 1; if (Q.cta_first[mid] <= a0) lo = mid; else hi = mid; }
+          b0 = lo; lo = b0; hi = gridDim.x;
+          while (hi - lo > 1u) { const uint32_t mid = (lo + hi) >> 1; if (Q.cta_first[mid] <= a1) lo = mid; else hi = mid; }
+          b1 = lo;
+        }
+        for (uint32_t b = b0; b <= b1; ++b)
+          if (b != blockIdx.x) atomicOr(&s_nbmap[b >> 5], 1u << (b & 31));
+      }
+    }
+    __syncthreads();
+  }
+
+  uint32_t tile_cap = (uint32_t)Q.tile_cells;     // halved (for the rest of this CTA's share) when a tile's neighbour pool overflows
+#pragma unroll 1
+  for (int pass = 0; pass < Q.npass; ++pass) {
+  const uint32_t colour = Q.npass > 1 ? Q.colours[pass] : A.colour;
+  const int px = colour & 1, py = (colour >> 1) & 1, pz = (colour >> 2) & 1;
+  const uint32_t colw = colour << 8;
+  const uint32_t c3dep = P_DEPPOS + colw;
+  bool must_wait = pass > 0;                      // pass 0 follows the cell build in stream order
   for (uint32_t cur = cta_lo; cur < cta_hi;) {
-    const uint32_t tile_n = min((uint32_t)Q.tile_cells, cta_hi - cur);
+    const uint32_t tile_n = min(tile_cap, cta_hi - cur);
     const uint32_t tile_lo = cur;
     cur += tile_n;
     if (t == 0) { s_scal[0] = 0; s_scal[1] = 0; s_scal[3] = 0; s_scal[4] = 0; s_scal[7] = 0; }
+    if (t < 4) s_tcnt[t] = 0u;
     __syncthreads();
 
     // ================================================================ phase 1a: one thread per active cell
@@ -317,16 +405,16 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
           if (!rot) {
             r1 = V3{wrap1(g, r0.x + A.d_max * sym_unit_bits(rm.x)), wrap1(g, r0.y + A.d_max * sym_unit_bits(rm.y)),
                     wrap1(g, r0.z + A.d_max * sym_unit_bits(rm.z))};
-            atomicAdd(&s_cnt[C_TRIALS_TRANS], 1u);
+            atomicAdd(&s_tcnt[0], 1u);
           } else {
             const V3 v = ball_sample(A.key, pid, 0, 0, P_MOVE + colw + (1u << 16), A.a_max, A.a_max2, n_blocks);
             q1 = rotate_cayley(q0, v);
-            atomicAdd(&s_cnt[C_TRIALS_ROT], 1u);
+            atomicAdd(&s_tcnt[1], 1u);
           }
           const int jx = cell_axis(g, r1.x, A.sx), jy = cell_axis(g, r1.y, A.sy), jz = cell_axis(g, r1.z, A.sz);
           if (jx != ix || jy != iy || jz != iz) {        // confinement (L180)
             A.outcome[pid] = (uint8_t)OUT_BOUNDARY;
-            atomicAdd(&s_cnt[C_REJ_BOUNDARY], 1u);
+            atomicAdd(&s_tcnt[2], 1u);
           } else {
             const uint32_t e = atomicAdd(&s_scal[4], 1u);
             s_r1[e] = make_float4(r1.x, r1.y, r1.z, p0.w);
@@ -349,6 +437,27 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
           }
         }
       }
+    }
+    // ---- passes after the first: the neighbourhood walk reads cells that neighbouring CTAs wrote in the previous
+    // pass (and they must be done reading ours): wait for their published pass counter.  Acquire loads by the
+    // polling threads + the barrier make their writes visible to the whole CTA.  Phase 1a above touched only this
+    // CTA's own cells, so it ran ahead of the wait.  Bounded spin: a stuck neighbour raises the error flag instead of a hang.
+    if (must_wait) {
+      must_wait = false;
+      const uint32_t target = Q.seq0 + (uint32_t)pass;
+      bool polled = false;
+      for (uint32_t b = (uint32_t)t; b < gridDim.x; b += T) {
+        if (!((s_nbmap[b >> 5] >> (b & 31)) & 1u)) continue;
+        uint32_t v, spins = 0;
+        for (;;) {       // relaxed polls (no L1 invalidation while spinning), one acquire fence at the end
+          asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(Q.done + b) : "memory");
+          if ((int32_t)(v - target) >= 0) break;
+          if (++spins > (1u << 22)) { atomicExch(A.err_flag, 2); break; }
+          __nanosleep(40);
+        }
+        polled = true;
+      }
+      if (polled) __threadfence();
     }
     __syncthreads();
     const int nlist = (int)s_scal[4];
@@ -411,7 +520,7 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
           if (!(r2 < Q.rlist2)) continue;
           if (!ANISO && r2 < g.dcirc2) { s_state[e] = OUT_HARD; continue; }     // a6 (spheres)
           const int pe = (int)atomicAdd(&s_scal[1], 1u);
-          if (pe >= POOL) { atomicExch(A.err_flag, 1); continue; }
+          if (pe >= POOL) continue;            // the tile is split and redone below (nothing is committed before that)
           const int prev = atomicExch(&s_head[e], pe);
           s_pool[pe * E] = make_float4(rho.x, rho.y, rho.z, __int_as_float(prev));
           if (ANISO) {
@@ -446,6 +555,12 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
       }
     }
     __syncthreads();
+    // ---- neighbour pool overflow (a locally dense tile, e.g. a cluster in a dilute box): nothing of this tile is
+    // committed yet (boundary outcomes are idempotent, its counters are tile-local), so halve the tile and redo it
+    if (s_scal[1] > (uint32_t)POOL) {
+      if (tile_n > 1u) { tile_cap = max(1u, tile_n >> 1); cur = tile_lo; __syncthreads(); continue; }
+      if (t == 0) atomicExch(A.err_flag, 1);     // ONE move with more listed neighbours than the whole pool holds
+    }
     // ================================================================ phase 1d: N_d by table inversion (a7)
 #pragma unroll 1
     for (int e = t; e < nlist; e += T) {
@@ -457,10 +572,11 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
         const unsigned long long U = ((unsigned long long)rn.x << 32) | rn.y;
         Nd = A.pt_klo + poisson_count(A.ptable, A.pt_n, Q.pguide, U);
       }
-      s_Nd[e] = Nd; s_knext[e] = 0; s_rejmin[e] = 0xffffffffu;
+      s_Nd[e] = Nd; s_knext[e] = 0; s_rejmin[e] = Nd;        // rejmin: smallest rejecting k so far, N_d = none
       if (s_state[e] == OUT_NONE && Nd != 0) s_alive[atomicAdd(&s_scal[0], 1u)] = (uint16_t)e;
     }
     __syncthreads();
+    if (!CB) {
     const int nalive = (int)s_scal[0];
     for (int w = t; w < NW; w += T) {
       const int rem = nalive - 32 * w;
@@ -471,10 +587,107 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
     {
       QTables tb;
       tb.r1 = s_r1; tb.rho = s_rho; tb.aold = s_aold; tb.anew = s_anew; tb.pool = s_pool;
-      tb.Nd = s_Nd; tb.knext = s_knext; tb.rejmin = s_rejmin; tb.head = s_head; tb.todo = s_todo; tb.alive = s_alive;
-      q_depletant_queue<SHAPE>(tb, nalive, g, A.key, c3dep, t, n_eval, n_blocks);
+      tb.knext = s_knext; tb.rejmin = s_rejmin; tb.head = s_head; tb.todo = s_todo; tb.alive = s_alive;
+      q_depletant_queue<SHAPE, false>(tb, nalive, g, A.key, c3dep, t, n_eval, n_blocks);
     }
     __syncthreads();
+    } else {
+    // ================================================================ phase 2 + 3: configurational bias (a8 + a9, Eq. 16)
+    // Rounds over windows of W depletant indices per move.  Round: (A) the item queue examines k in [k_lo, k_lo + W)
+    // of every running move; rejecting depletants become jobs.  (B) the 2 n_trial reinsertions of every job are items
+    // (job, t, dir) spread over the lanes; counts by shared atomics.  (C) one thread per move folds its jobs in
+    // ASCENDING k into the fp32 product (the order is part of the definition) and stops at the first zero weight
+    // (R-G3), which also fixes dep_needed and the reinsertion count exactly as the sequential definition does.
+    const uint32_t ne = 2u * (uint32_t)A.n_trial;
+    const uint32_t c3cb = P_CBPOS + colw;
+    uint32_t W = HPMC_CB_WINDOW;
+    for (int e = t; e < nlist; e += T) { s_P[e] = 1.0f; s_cbre[e] = 0u; s_klo[e] = 0u; }
+    __syncthreads();
+    for (;;) {
+      if (t == 0) { s_scal[0] = 0; s_scal[5] = 0; }
+      __syncthreads();
+      for (int e = t; e < nlist; e += T) {
+        const uint32_t klo = s_klo[e], Nd = s_Nd[e];
+        if (s_state[e] == OUT_NONE && klo < Nd) {
+          s_alive[atomicAdd(&s_scal[0], 1u)] = (uint16_t)e;
+          s_knext[e] = klo; s_rejmin[e] = min(Nd, klo + W); s_jhead[e] = -1;
+        }
+      }
+      __syncthreads();
+      const int nalive = (int)s_scal[0];
+      if (nalive == 0) break;
+      for (int w = t; w < NW; w += T) {
+        const int rem = nalive - 32 * w;
+        s_todo[w] = rem >= 32 ? 0xffffffffu : (rem > 0 ? ((1u << rem) - 1u) : 0u);
+      }
+      __syncthreads();
+      {
+        QTables tb;
+        tb.r1 = s_r1; tb.rho = s_rho; tb.aold = s_aold; tb.anew = s_anew; tb.pool = s_pool;
+        tb.knext = s_knext; tb.rejmin = s_rejmin; tb.head = s_head; tb.todo = s_todo; tb.alive = s_alive;
+        tb.jk = s_jk; tb.jm = s_jm; tb.jc = s_jc; tb.jhead = s_jhead; tb.njobs = &s_scal[5]; tb.jcap = S::JCAP;
+        q_depletant_queue<SHAPE, true>(tb, nalive, g, A.key, c3dep, t, n_eval, n_blocks);
+      }
+      __syncthreads();
+      const uint32_t njobs = s_scal[5];
+      if (njobs > (uint32_t)S::JCAP) {       // more rejecting depletants than job slots: redo the round with half the window
+        W = max(1u, W >> 1);                 // (W = 1 gives at most one job per move: always fits)
+        __syncthreads();
+        continue;
+      }
+      // ---- (B) reinsertion items
+      const uint32_t nitems = njobs * ne;
+#pragma unroll 1
+      for (uint32_t i = t; i < nitems; i += T) {
+        const uint32_t jb = i / ne, e2 = i - jb * ne;
+        const uint32_t m = s_jm[jb] & 0xffffu, kk = s_jk[jb];
+        const uint32_t dir = e2 & 1u, tt = e2 >> 1;
+        const float4 r1f = s_r1[m], rof = s_rho[m];
+        const V3 ro = V3{rof.x, rof.y, rof.z};
+        V3 ao = V3{0.f, 0.f, 1.f}, an = V3{0.f, 0.f, 1.f};
+        if (ANISO) { const float4 a0 = s_aold[m], a1 = s_anew[m]; ao = V3{a0.x, a0.y, a0.z}; an = V3{a1.x, a1.y, a1.z}; }
+        V3 sp = ball_sample(A.key, __float_as_uint(r1f.w), kk, tt + (dir << 16), c3cb, g.Rins, g.Rins2, n_blocks);
+        bool valid;
+        if (dir == 0) {                  // forward: about the old centre, must overlap the old pose only (R-G2)
+          sp = sp + ro;
+          valid = dep_overlap<SHAPE>(g, sp - ro, ao) && !dep_overlap<SHAPE>(g, sp, an);
+        } else {                         // reverse: about the new centre, must overlap the new pose only
+          valid = q_new_only<SHAPE>(g, sp, ro, ao, an);
+        }
+        if (valid) {
+          const bool fr = q_free_of_nbrs<SHAPE>(g, s_pool, s_head[m], sp);
+          atomicAdd(dir == 0 ? &s_jc[jb].x : &s_jc[jb].y, fr ? 0x10001u : 1u);
+        }
+      }
+      __syncthreads();
+      // ---- (C) fold the jobs of every running move in ascending k
+#pragma unroll 1
+      for (int j = t; j < nalive; j += T) {
+        const uint32_t e = s_alive[j];
+        float P = s_P[e];
+        uint32_t cbre = s_cbre[e];
+        long long last = -1;
+        bool zero = false;
+        for (;;) {
+          int best = -1; uint32_t bk = 0xffffffffu;
+          for (int jb = s_jhead[e]; jb >= 0; jb = (int)(s_jm[jb] >> 16) - 1) {
+            const uint32_t kk = s_jk[jb];
+            if ((long long)kk > last && kk < bk) { bk = kk; best = jb; }
+          }
+          if (best < 0) break;
+          last = (long long)bk;
+          const uint2 c = s_jc[best];
+          const uint32_t Ni = c.x & 0xffffu, Npins = c.x >> 16, Npi = c.y & 0xffffu, Nins = c.y >> 16;
+          ++cbre;
+          if (Npins == 0u) { zero = true; s_state[e] = OUT_CB; s_rejmin[e] = bk + 1u; break; }   // R-G3; dep_needed = k + 1
+          P = P * __fdiv_rn((float)(Npins * (Npi + 1u)), (float)((Nins + 1u) * Ni));            // Eq. 16, R-G1
+        }
+        s_P[e] = P; s_cbre[e] = cbre;
+        if (!zero) s_klo[e] = s_rejmin[e];     // window end
+      }
+      __syncthreads();
+    }
+    }
     // ================================================================ commit (a10)
 #pragma unroll 1
     for (int e = t; e < nlist; e += T) {
@@ -482,12 +695,26 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
       const float4 r1f = s_r1[e];
       const uint32_t pid = __float_as_uint(r1f.w);
       const bool rot = (s_cell[e] >> 30) & 1u;
-      if (out == OUT_NONE) {
+      if (!CB && out == OUT_NONE) {
         const uint32_t Nd = s_Nd[e], rm_ = s_rejmin[e];
         const bool rej = rm_ < Nd;
         out = rej ? OUT_DEPLETANT : OUT_ACCEPT;
         atomicAdd(&s_cnt[C_DEP_DRAWN], Nd);
         atomicAdd(&s_cnt[C_DEP_NEEDED], rej ? rm_ + 1u : Nd);
+      }
+      if (CB && (out == OUT_NONE || out == OUT_CB)) {
+        const uint32_t Nd = s_Nd[e], cbre = s_cbre[e];
+        atomicAdd(&s_cnt[C_DEP_DRAWN], Nd);
+        atomicAdd(&s_cnt[C_DEP_NEEDED], out == OUT_CB ? s_rejmin[e] : Nd);
+        if (cbre) atomicAdd(&s_cnt[C_CB_REINSERTIONS], cbre * 2u * (uint32_t)A.n_trial);
+        if (out == OUT_NONE) {
+          if (cbre == 0u) out = OUT_ACCEPT;          // no rejecting depletant at all
+          else {
+            const Block4 ra = philox(A.key, pid, 0, 0, P_ACCEPT + colw);
+            ++n_blocks;
+            out = (unit01(ra.x) < s_P[e]) ? OUT_ACCEPT : OUT_CB;
+          }
+        }
       }
       A.outcome[pid] = (uint8_t)out;
       if (out == OUT_ACCEPT) {
@@ -502,10 +729,25 @@ __global__ void __launch_bounds__(T, QLayout<SHAPE>::MIN_CTAS) k_moveq(const QAr
           A.caxis[slot] = make_float4(an.x, an.y, an.z, 0.0f);
         }
         atomicAdd(&s_cnt[rot ? C_ACCEPT_ROT : C_ACCEPT_TRANS], 1u);
-      } else atomicAdd(&s_cnt[out == OUT_HARD ? C_REJ_HARD : C_REJ_DEPLETANT], 1u);
+      } else atomicAdd(&s_cnt[out == OUT_HARD ? C_REJ_HARD : (out == OUT_CB ? C_REJ_CB : C_REJ_DEPLETANT)], 1u);
+    }
+    if (t == 0) {
+      atomicAdd(&s_cnt[C_TRIALS_TRANS], s_tcnt[0]); atomicAdd(&s_cnt[C_TRIALS_ROT], s_tcnt[1]);
+      atomicAdd(&s_cnt[C_REJ_BOUNDARY], s_tcnt[2]);
     }
     __syncthreads();
   }
+  // ---- publish the pass: every commit of this CTA is ordered before the counter by the barrier above + the release
+  if (Q.npass > 1) {
+    if (must_wait) {      // a CTA without cells in this pass still has to respect the order of its neighbours' passes: nothing to do
+      must_wait = false;
+    }
+    if (t == 0) {
+      const uint32_t v = Q.seq0 + (uint32_t)pass + 1u;
+      asm volatile("st.release.gpu.global.u32 [%0], %1;" :: "l"(Q.done + blockIdx.x), "r"(v) : "memory");
+    }
+  }
+  }   // pass
 
   // ---- counters: REDUX for the two register counters, then one global atomic per CTA and counter
   {

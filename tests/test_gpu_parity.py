@@ -3,8 +3,9 @@ on the same seeded inputs.  Bar (BASELINE.json north_star): per-move outcome cod
 after every sweep; integer counters that both sides define (everything except dep_evaluated / philox_blocks,
 which describe each implementation's own work) equal.
 
-Default sweep counts keep the suite to a few minutes; HPMC_PARITY_FULL=1 runs the configs' full lengths
-(min(1000, sweeps) per north_star).
+The default runs the configs' full lengths (min(1000, sweeps) per north_star: C1 100, C2 4 x 1000, C3 200 at
+1,048,576 spheres, C4 500, C5 500 sweeps; about 80 s on a B200 box with 16 host cores for the oracle).
+HPMC_PARITY_SHORT=1 shortens them for local iterations.
 """
 import os
 
@@ -15,7 +16,7 @@ import workloads
 
 pytestmark = pytest.mark.gpu
 
-FULL = os.environ.get("HPMC_PARITY_FULL", "0") == "1"
+FULL = os.environ.get("HPMC_PARITY_SHORT", "0") != "1"
 SHARED_COUNTERS = ("trials_trans", "accept_trans", "trials_rot", "accept_rot", "rej_boundary", "rej_hard",
                    "rej_depletant", "rej_cb", "dep_drawn", "dep_needed", "cb_reinsertions")
 
@@ -126,6 +127,30 @@ def test_c5_spherodisks_configurational_bias():
     pos, quat = workloads.generate(cfg)
     c = run_parity(cfg, pos, quat, 500 if FULL else 30, cfg.n_R())
     assert c["cb_reinsertions"] > 0 and c["rej_cb"] > 0 and c["accept_rot"] > 0
+
+
+@pytest.mark.parametrize("name,N,n_trial,sweeps", [("C5", None, 4, 120), ("C5", 4096, 40, 40), ("C1", None, 10, 100),
+                                                   ("C4", 4096, 3, 40)])
+def test_configurational_bias_through_the_item_queue_kernel(monkeypatch, name, N, n_trial, sweeps):
+    """The CB stage of the item-queue kernel (HPMC_CB_KERNEL=queue: windows of depletant indices, reinsertion items,
+    product folded in ascending k): C5 itself, a large n_trial (PAPER.md L228 recommends n_trial >~ 10), and CB on
+    spheres and half-balls."""
+    import dataclasses
+    monkeypatch.setenv("HPMC_CB_KERNEL", "queue")
+    cfg = dataclasses.replace(workloads.config(name, N), n_trial=n_trial)
+    pos, quat = workloads.generate(cfg)
+    c = run_parity(cfg, pos, quat, sweeps if FULL else 15, cfg.n_R())
+    assert c["cb_reinsertions"] > 0 and c["rej_cb"] > 0
+
+
+def test_one_launch_per_pass_mode(monkeypatch):
+    """HPMC_SWEEP_LAUNCHES=8: the item-queue kernel launched once per checkerboard pass (no neighbour waits) instead of
+    once per sweep; same bits."""
+    monkeypatch.setenv("HPMC_SWEEP_LAUNCHES", "8")
+    for name, N, sweeps in (("C3", 65536, 10), ("C4", 4096, 10)):
+        cfg = workloads.config(name, N)
+        pos, quat = workloads.generate(cfg)
+        run_parity(cfg, pos, quat, sweeps, cfg.n_R())
 
 
 def test_c5_dense_after_compression_hard_overlaps():
@@ -248,6 +273,51 @@ def test_dense_fcc_crystal_neighbour_pool():
     c = run_parity(cfg, pos, None, 3, cfg.n_R(), check_cells_every=1)
     assert c["rej_hard"] > 0
 
+
+
+def _clustered_slab(cfg, frac=1.0 / 3.0):
+    """The paper's use case is depletion-driven aggregation (Fig. 7): a dense fcc slab (phi = 0.66
+    locally) filling a third of the box along z, the rest empty.  Positions only; no arithmetic of the method."""
+    L = cfg.box_L
+    nn = (4.0 * (np.pi / 6.0) / 0.66) ** (1.0 / 3.0) / np.sqrt(2.0)      # nearest-neighbour distance of fcc at phi = 0.66
+    a = nn * np.sqrt(2.0)
+    ncx = int(L / a)
+    ncz = int(frac * L / a)
+    ax, az = L / ncx, a                                                   # stretched to fit the box in x, y (periodic)
+    base = np.array([(0, 0, 0), (0.5, 0.5, 0), (0.5, 0, 0.5), (0, 0.5, 0.5)], np.float64)
+    ii, kk = np.arange(ncx), np.arange(ncz)
+    g = np.stack(np.meshgrid(ii, ii, kk, indexing="ij"), -1).reshape(-1, 1, 3) + base[None]
+    pos = g.reshape(-1, 3) * np.array([ax, ax, az]) + 0.25 * a
+    assert ax / np.sqrt(2.0) > 1.0005 * cfg.sigma_c
+    p4 = np.zeros((len(pos), 4), np.float32)
+    p4[:, :3] = pos
+    assert p4[:, :3].max() < np.float32(L)
+    return p4
+
+
+def test_clustered_slab_neighbour_pool_recovers():
+    """A clustered system at low MEAN density (the paper's aggregation use case, L218): a close-packed slab in a
+    C3-sized box, ~8e5 spheres with 12 listed neighbours each where the box average suggests ~5.  The move kernel
+    must split tiles whose neighbour pool overflows and stay bit-exact (no HPMC_E_NEIGHBOR_OVERFLOW)."""
+    import dataclasses
+    cfg = dataclasses.replace(workloads.config("C3"), q=0.08, d_max=0.03, phi_d_r=(0.1,))
+    pos = _clustered_slab(cfg)
+    cfg = dataclasses.replace(cfg, N=len(pos), phi_c=len(pos) * (np.pi / 6) / cfg.box_L ** 3)
+    assert cfg.N >= 500000 and abs(cfg.box_L - workloads.config("C3").box_L) < 1e-3
+    c = run_parity(cfg, pos, None, 3, cfg.n_R(), check_cells_every=1)
+    assert c["rej_hard"] > 0 and c["rej_depletant"] > 0
+
+
+def test_clustered_slab_large_tiles_forced(monkeypatch):
+    """The same slab with the tile size forced far above what the pool holds: every tile of the slab overflows and
+    is split (several times) inside the CTA."""
+    import dataclasses
+    monkeypatch.setenv("HPMC_CELLS_PER_CTA", "400")
+    monkeypatch.setenv("HPMC_POOL_CAP_OFF", "1")
+    cfg = dataclasses.replace(workloads.config("C3"), q=0.08, d_max=0.03, phi_d_r=(0.1,))
+    pos = _clustered_slab(cfg, frac=0.12)
+    cfg = dataclasses.replace(cfg, N=len(pos), phi_c=len(pos) * (np.pi / 6) / cfg.box_L ** 3)
+    run_parity(cfg, pos, None, 2, cfg.n_R(), check_cells_every=1)
 
 
 @pytest.mark.parametrize("cells_per_cta,tile", [(600, 64), (None, 64)])
