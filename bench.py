@@ -28,18 +28,50 @@ if ROOT not in sys.path:
 
 import workloads  # noqa: E402
 
-# Algorithmic work per unit: lane-operations (one thread executing one plain ALU instruction).
-OPS_PER_NEEDED_DEPLETANT = 131.0   # 1.91 attempts x (40 INT Philox + 22 convert/scale/|d|^2/compare) + 11 pose tests + ~2 nbr
-OPS_PER_MOVE = 500.0               # 3 Philox blocks, 27-cell staging, hard overlap, table search, commit
+# Algorithmic work per unit, in lane-operations (one thread executing one plain ALU instruction).  The table is
+# frozen in BASELINE.md section 3 (derivation: DESIGN.md section 6); it multiplies the COUNTERS of the timed run
+# (dep_needed, trials, cb_reinsertions), never what the kernel happened to execute.
+#   per Philox block 40 (10 rounds x (2 wide multiplies + 2 three-input XORs)); per cube-rejection attempt 62 (block +
+#   3 x bits->float/scale + |d|^2 + compare); attempts per depletant 6/pi = 1.91
+OPS_PER_NEEDED_DEPLETANT = {"sphere": 131.0,      # 1.91 x 62 + old/new pose tests 11 + ~2 neighbour tests
+                            "halfball": 167.0,    # + 15 + 15 closed-form new/old tests + 0.07 n_nbr x 25
+                            "spherodisk": 167.0}
+OPS_PER_MOVE = {"sphere": 500.0,                  # 3 Philox blocks, 27-cell walk (~20 candidates x 12 + 9 rows x 8), table search, commit
+                "halfball": 1500.0,               # + axis staging, ~2 support-function pair tests of ~400 ops (a6)
+                "spherodisk": 1500.0}
+OPS_PER_CB_REINSERTION = {"sphere": 150.0, "halfball": 190.0, "spherodisk": 190.0}   # 1.91 x 62 + both pose tests + neighbour tests
+PHILOX_BLOCKS_PER_DEPLETANT = 6.0 / 3.141592653589793
 BYTES_PER_PARTICLE_PER_PASS = 16.0 # every pass reads the cell-ordered float4 array once (re-reads by neighbouring cells are L2 hits)
 BYTES_PER_CELL_PER_PASS = 4.0      # ... and each cell_start word once
 BYTES_PER_MOVE = 1.0               # outcome code
 BYTES_PER_ACCEPT = 48.0
-# dram__bytes_read.sum + dram__bytes_write.sum of one move-kernel launch at C3, ncu --set full (profiles/r1f_summary.md:
-# 22.50 MB read + 0 written; capture d saw 2.8..4.9 MB of write-backs of the preceding build on top)
-NCU_TRAFFIC_BYTES_PER_LAUNCH_C3 = 22.5e6
-LANES_PER_SM_PER_CLK = 128.0       # 4 SMSPs x 32 lanes: issue-rate peak of the plain ALU pipes
-NUM_SMS = 148
+LANES_PER_SM_PER_CLK = 128.0       # 4 SMSPs x 32 lanes x 1 warp-instruction per clock: the issue bound (kept as peak_issue_bound)
+KERNEL_SOURCES = ("moveq.cuh", "move.cuh", "geometry.cuh", "philox.cuh", "cells.cuh", "hpmc_lib.cu")
+
+
+def kernel_sources_sha():
+    """sha256 over the CUDA sources: a stored ncu traffic figure is only quoted while the kernels are unchanged."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_1508_07077_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the move kernel from the tracked capture
+    profiles/ncu_traffic.json (written from an `ncu --set full` run; names the source hash it was taken at).  None if
+    there is no capture of THIS source state for this workload."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if not os.path.exists(path):
+        return None, None
+    with open(path) as f:
+        d = json.load(f)
+    e = d.get(workload)
+    if not e or e.get("kernel_sources_sha") != kernel_sources_sha():
+        return None, None
+    return float(e["dram_bytes_per_launch"]), e.get("source")
 
 
 def parse_args():
@@ -52,6 +84,7 @@ def parse_args():
     ap.add_argument("--n", type=int, default=None, help="override particle count (debug; invalidates the headline)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the short runs of C1, C2, C4, C5 (per_config)")
     return ap.parse_args()
 
 
@@ -180,6 +213,127 @@ def run_reference(args, cfg):
     print(json.dumps(line), flush=True)
 
 
+def roofline_block(cfg, c, n_c, passes, launches, kernel_ms, step_ms_total, alu, pk, clocks, workload_key):
+    """Roofline of the move kernel (K-B) from the counters `c` of the timed run and its event-timed duration.
+    The lower bound on its time is the larger of (a) the Philox blocks the algorithm needs divided by the MEASURED
+    block rate of the SMs (the wide-multiply pipe binds a Philox stream: hpmc_alu_peaks) and (b) all algorithmic
+    lane-operations divided by the measured two-pipe issue rate; `peak` is the lane-op rate that bound corresponds to."""
+    moves = c["trials_trans"] + c["trials_rot"]
+    alg_ops = (c["dep_needed"] * OPS_PER_NEEDED_DEPLETANT[cfg.shape] + moves * OPS_PER_MOVE[cfg.shape]
+               + c["cb_reinsertions"] * OPS_PER_CB_REINSERTION[cfg.shape])
+    blocks = ((c["dep_needed"] + c["cb_reinsertions"]) * PHILOX_BLOCKS_PER_DEPLETANT + 3.0 * moves)
+    alg_bytes = (passes * (BYTES_PER_PARTICLE_PER_PASS * cfg.N * (1 if cfg.shape == "sphere" else 2)
+                           + BYTES_PER_CELL_PER_PASS * (n_c ** 3 + 1))
+                 + moves * BYTES_PER_MOVE + (c["accept_trans"] + c["accept_rot"]) * BYTES_PER_ACCEPT)
+    kernel_s = kernel_ms * 1e-3
+    sms, hz = alu["num_sms"], pk["sm_max_mhz"] * 1e6
+    t_philox = blocks / (alu["philox_blocks_ilp4"] * sms * hz)
+    t_issue = alg_ops / (alu["fadd_lop3_mix"] * sms * hz)
+    t_hbm = alg_bytes / (pk["hbm_gbs"] * 1e9)
+    t_alu = max(t_philox, t_issue)
+    peak = alg_ops / t_alu
+    ach = alg_ops / kernel_s if kernel_s > 0 else 0.0
+    hbm_ach = alg_bytes / kernel_s / 1e9 if kernel_s > 0 else 0.0
+    issue_peak = sms * LANES_PER_SM_PER_CLK * hz
+    seen_mhz = clocks.get("sm_mhz") or pk["sm_max_mhz"]
+    traffic, traffic_src = ncu_traffic(workload_key)
+    cb_warp = cfg.n_trial > 0 and os.environ.get("HPMC_CB_KERNEL") != "queue"
+    kern = ("k_move<%s,cb> (warp per cell, 8 launches per sweep)" % cfg.shape if cb_warp else
+            "k_moveq<%s,%s> (item queue, %d launch%s per sweep)" % (cfg.shape, "cb" if cfg.n_trial > 0 else "plain",
+                                                                     round(launches / max(1, passes / 8)),
+                                                                     "" if launches * 8 == passes else "es"))
+    return {
+        "bound": "alu" if t_alu >= t_hbm else "hbm",
+        "achieved": ach / 1e12, "peak": peak / 1e12, "unit": "Tlaneop/s", "frac": t_alu / kernel_s if kernel_s > 0 else None,
+        "frac_cycles": (t_alu * hz) / (kernel_s * seen_mhz * 1e6) if kernel_s > 0 else None,
+        "traffic": traffic, "traffic_source": traffic_src,
+        "peak_source": "measured live: hpmc_alu_peaks on this device (per SM per clock: %.3f Philox blocks, %.1f lane-ops two-pipe "
+                       "issue) x %d SMs x %.0f MHz; binding term: %s; HBM %s" % (
+                           alu["philox_blocks_ilp4"], alu["fadd_lop3_mix"], sms, pk["sm_max_mhz"],
+                           "philox pipe" if t_philox >= t_issue else "issue", pk["source"]),
+        "peak_issue_bound": issue_peak / 1e12, "frac_of_issue_bound": ach / issue_peak,
+        "alg_laneops_per_launch": alg_ops / max(1, launches), "alg_philox_blocks_per_launch": blocks / max(1, launches),
+        "alg_bytes_per_launch": alg_bytes / max(1, launches),
+        "kernel": kern, "launches": launches, "passes": passes, "avg_launch_ms": kernel_ms / max(1, launches),
+        "us_per_pass": 1e3 * kernel_ms / max(1, passes),
+        "share_of_step": kernel_ms / step_ms_total if step_ms_total else None,
+        "hbm": {"achieved": hbm_ach, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": hbm_ach / pk["hbm_gbs"]},
+        "alg_ops_per_needed_depletant": OPS_PER_NEEDED_DEPLETANT[cfg.shape], "alg_ops_per_move": OPS_PER_MOVE[cfg.shape],
+        "alg_ops_per_cb_reinsertion": OPS_PER_CB_REINSERTION[cfg.shape],
+    }
+
+
+def timed_run(hp, torch, cfg, seed, pos, quat, n_R, steps, warmup, flush, step0=0):
+    """`warmup` untimed + `steps` timed sweeps of one configuration from the given poses; returns the counters of the
+    timed sweeps, per-step event times, the move kernel's event time and launch count, the grid size."""
+    dpos = torch.from_numpy(pos.copy()).cuda()
+    dquat = None if quat is None else torch.from_numpy(quat.copy()).cuda()
+    h = hp.HPMC(cfg.shape, cfg.sigma_c, cfg.sigma_d, cfg.box_L, cfg.d_max, dpos, dquat, cfg.disk_a, cfg.disk_s)
+
+    def step(s):
+        h.build_cells(seed, s)
+        h.sweep(seed, s, n_R, cfg.d_max, cfg.a_max, cfg.n_trial)
+
+    for s in range(warmup):
+        step(step0 + s)
+    torch.cuda.synchronize()
+    h.reset_counters()
+    l0 = h.launch_count()
+    h.time_move_kernel(True)
+    starts = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+    ends = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+    torch.cuda.synchronize()
+    for k in range(steps):
+        if flush is not None:
+            flush.zero_()                  # evict the working set from L2 between timed steps (not timed)
+        starts[k].record()
+        step(step0 + warmup + k)
+        ends[k].record()
+    torch.cuda.synchronize()
+    step_ms = [a.elapsed_time(b) for a, b in zip(starts, ends)]
+    kms, kl = h.move_kernel_ms()
+    h.time_move_kernel(False)
+    c = h.counters()
+    out = dict(c=c, step_ms=step_ms, kernel_ms=kms, kernel_launches=kl, launches=h.launch_count() - l0, n_c=h.n_c,
+               final_pos=dpos.cpu().numpy(), final_quat=None if dquat is None else dquat.cpu().numpy())
+    h.close()
+    return out
+
+
+def per_config_lines(hp, torch, alu, pk, flush, clocks):
+    """moves/s, depletant insertions/s, us per pass and roofline fraction of the other BASELINE.json configurations
+    (C1, C2 at its four reservoir densities after melting 1000 sweeps at n_R = 0 through the library, C4, C5), each a
+    short device-timed run from its seeded initial state.  Context for the C3 headline, same kernels, same clocks."""
+    out = {}
+    plan = [("C1", None, 200), ("C2", None, 50), ("C4", None, 50), ("C5", None, 50)]
+    for name, _, steps in plan:
+        cfg = workloads.config(name)
+        pos, quat = workloads.generate(cfg)
+        dens = [(None, cfg.n_R())]
+        if name == "C2":
+            m = timed_run(hp, torch, cfg, cfg.seed, pos, quat, 0.0, 1000, 0, None, step0=100000)   # melt (configs[1])
+            pos = m["final_pos"]
+            dens = [(phi, cfg.n_R(phi)) for phi in cfg.phi_d_r]
+        for phi, n_R in dens:
+            r = timed_run(hp, torch, cfg, cfg.seed, pos, quat, n_R, steps, 5, flush)
+            c = r["c"]
+            tot_s = sum(r["step_ms"]) * 1e-3
+            moves = c["trials_trans"] + c["trials_rot"]
+            rf = roofline_block(cfg, c, r["n_c"], 8 * steps, r["kernel_launches"], r["kernel_ms"], sum(r["step_ms"]), alu, pk,
+                                clocks, name)
+            key = name if phi is None else "%s phi_d^r=%.1f" % (name, phi)
+            out[key] = {
+                "workload": workload_desc(cfg) if phi is None else workload_desc(cfg).replace(
+                    "phi_d^r=%.2f" % cfg.phi_d_r[0], "phi_d^r=%.2f" % phi),
+                "moves_per_s": moves / tot_s, "dep_needed_per_s": c["dep_needed"] / tot_s,
+                "dep_evaluated_per_s": c["dep_evaluated"] / tot_s, "dep_drawn_per_s": c["dep_drawn"] / tot_s,
+                "ms_per_step": 1e3 * tot_s / steps, "us_per_pass": rf["us_per_pass"], "acceptance":
+                (c["accept_trans"] + c["accept_rot"]) / max(1, moves), "roofline_frac": rf["frac"],
+                "frac_of_issue_bound": rf["frac_of_issue_bound"], "kernel": rf["kernel"], "steps": steps,
+            }
+    return out
+
+
 def main():
     args = parse_args()
     cfg = workloads.config(args.workload, args.n)
@@ -198,6 +352,8 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     pk = peaks()
+    hp.alu_peaks()                         # warm-up of the micro-benchmark (clocks, instruction cache)
+    alu = hp.alu_peaks()                   # measured ALU pipe rates of THIS device (per SM per clock)
 
     # replicas only: every rank runs the same configuration from its own seeded input
     import dataclasses
@@ -276,25 +432,11 @@ def main():
         hh.close()
 
     if rank == 0:
-        alg_ops = c["dep_needed"] * OPS_PER_NEEDED_DEPLETANT + moves * OPS_PER_MOVE
-        alg_bytes = (move_launches * (BYTES_PER_PARTICLE_PER_PASS * cfg.N + BYTES_PER_CELL_PER_PASS * (h.n_c ** 3 + 1))
-                     + moves * BYTES_PER_MOVE + (c["accept_trans"] + c["accept_rot"]) * BYTES_PER_ACCEPT)
-        move_s = move_ms * 1e-3
-        alu_peak = NUM_SMS * LANES_PER_SM_PER_CLK * pk["sm_max_mhz"] * 1e6          # lane-ops/s at max boost clock
-        alu_ach = alg_ops / move_s if move_s > 0 else 0.0
-        hbm_ach = alg_bytes / move_s / 1e9 if move_s > 0 else 0.0
-        t_alu, t_hbm = alg_ops / alu_peak, alg_bytes / (pk["hbm_gbs"] * 1e9)
-        roofline = {
-            "bound": "alu" if t_alu >= t_hbm else "hbm",
-            "achieved": alu_ach / 1e12, "peak": alu_peak / 1e12, "unit": "Tlaneop/s", "frac": alu_ach / alu_peak,
-            "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH_C3 if (cfg.name == "C3" and args.n is None) else None,
-            "alg_bytes_per_launch": alg_bytes / max(1, move_launches), "alg_laneops_per_launch": alg_ops / max(1, move_launches),
-            "kernel": "k_moveq (8 launches per step)", "launches": move_launches,
-            "avg_launch_ms": move_ms / max(1, move_launches), "share_of_step": move_ms / total_ms if total_ms else None,
-            "peak_source": "derived: 148 SM x 128 lanes/clk x %.0f MHz (DESIGN.md); HBM %s" % (pk["sm_max_mhz"], pk["source"]),
-            "hbm": {"achieved": hbm_ach, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": hbm_ach / pk["hbm_gbs"]},
-            "alg_ops_per_needed_depletant": OPS_PER_NEEDED_DEPLETANT, "alg_ops_per_move": OPS_PER_MOVE,
-        }
+        wkey = cfg.name if args.n is None else None
+        roofline = roofline_block(cfg, c, h.n_c, 8 * args.steps, move_launches, move_ms, total_ms, alu, pk, clocks, wkey)
+        per_config = None
+        if not args.no_per_config and world == 1 and cfg.name == "C3" and args.n is None:
+            per_config = per_config_lines(hp, torch, alu, pk, flush, clocks)
         cpu = None
         if not args.no_cpu_baseline and world == 1:
             # bounded sample: about 12 s of oracle time on this box's cores (3 sweeps at least, 2000 at most)
@@ -313,8 +455,8 @@ def main():
                        "moves_per_step": g_moves / args.steps / world},
             "depletant_insertions_per_s": {"evaluated": g_eval / tot_s, "needed": g_needed / tot_s, "drawn": g_drawn / tot_s},
             "acceptance": (c["accept_trans"] + c["accept_rot"]) / max(1, moves),
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-            "wall_s_timed_region": t_wall,
+            "roofline": roofline, "alu_peaks_per_sm_per_clk": alu, "cpu_baseline": cpu, "e2e": e2e,
+            "gpu_launches": launches, "clocks": clocks, "per_config": per_config, "wall_s_timed_region": t_wall,
         }
         print(json.dumps(line), flush=True)
     h.close()

@@ -377,14 +377,16 @@ int hpmc_init(hpmc_ctx** out, const hpmc_params* p, int64_t N, float* d_pos4, fl
   CUI(cudaMalloc(&ctx->d_cid, sizeof(uint32_t) * N));
   CUI(cudaMalloc(&ctx->d_rank, sizeof(uint32_t) * N));
   CUI(cudaMalloc(&ctx->d_cell_pid, sizeof(uint32_t) * N));
-  CUI(cudaMalloc(&ctx->d_counts, sizeof(uint32_t) * ctx->ncell));
-  CUI(cudaMalloc(&ctx->d_cell_start, sizeof(uint32_t) * ((size_t)ctx->ncell + 1)));
+  // counts and cell_start are padded to whole scan tiles (+ one tile for cell_start[ncell]): the scan kernels move uint4
+  const size_t padded = (size_t)ctx->ntiles * SCAN_TILE;
+  CUI(cudaMalloc(&ctx->d_counts, sizeof(uint32_t) * padded));
+  CUI(cudaMalloc(&ctx->d_cell_start, sizeof(uint32_t) * (padded + SCAN_TILE)));
   CUI(cudaMalloc(&ctx->d_tile_sums, sizeof(uint32_t) * (size_t)ctx->ntiles));
   CUI(cudaMalloc(&ctx->d_outcome, (size_t)N));
   CUI(cudaMalloc(&ctx->d_counters, sizeof(unsigned long long) * C_COUNT));
   CUI(cudaMalloc(&ctx->d_err, sizeof(int)));
   CUI(cudaMemsetAsync(ctx->d_outcome, 0, (size_t)N, ctx->stream));
-  CUI(cudaMemsetAsync(ctx->d_counts, 0, sizeof(uint32_t) * ctx->ncell, ctx->stream));   // kept zero between builds by k_scan_apply
+  CUI(cudaMemsetAsync(ctx->d_counts, 0, sizeof(uint32_t) * padded, ctx->stream));   // kept zero between builds by k_scan_apply
   CUI(cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * C_COUNT, ctx->stream));
   CUI(cudaMemsetAsync(ctx->d_err, 0, sizeof(int), ctx->stream));
 #undef CUI
