@@ -80,6 +80,10 @@ struct hpmc_ctx {
   bool use_queue = true;               // HPMC_MOVE_KERNEL=warp selects the first (warp-per-cell) design
   bool cb_queue = false;               // HPMC_CB_KERNEL=queue: configurational bias through the item-queue kernel too
   int64_t launches = 0;
+#ifdef HPMC_PHASE_CLOCKS
+  unsigned long long* d_phase_clk = nullptr;   // tuning build: per-phase clock sums of the move kernel (printed by hpmc_destroy)
+  int64_t phase_ctas = 0;
+#endif
   bool timing = false;
   std::vector<EventPair> ev;
   size_t ev_used = 0;
@@ -202,11 +206,20 @@ int get_table(hpmc_ctx* ctx, double lambda, PoissonTable** out) {
 constexpr int QT = HPMC_QT;                // threads per CTA of the item-queue kernel
 template <int SHAPE> struct QCfg { static constexpr int CPT = SHAPE == SH_SPHERE ? HPMC_QCPT : 1; };   // tile capacity CPT*QT cells
 
+// tuning builds only (HPMC_PHASE_CLOCKS): HPMC_SMEM_PAD bytes of unused dynamic shared memory lower the number of
+// resident CTAs per SM, to time a CTA's phases without its neighbours on the SM
+inline size_t smem_pad() {
+#ifdef HPMC_PHASE_CLOCKS
+  if (const char* o = getenv("HPMC_SMEM_PAD")) return (size_t)atol(o);
+#endif
+  return 0;
+}
+
 template <int SHAPE, bool CB>
 int setup_moveq(hpmc_ctx* ctx) {
   QPlan& P = ctx->plan[CB ? 1 : 0];
   using SM = QSmem<SHAPE, QT, QCfg<SHAPE>::CPT, CB>;
-  const size_t smem = SM::bytes;
+  const size_t smem = SM::bytes + smem_pad();
   cudaError_t e = cudaFuncSetAttribute(k_moveq<SHAPE, QT, QCfg<SHAPE>::CPT, CB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return fail(ctx, HPMC_E_CUDA, std::string("cudaFuncSetAttribute: ") + cudaGetErrorString(e));
   int per_sm = 0;
@@ -300,6 +313,10 @@ int launch_moveq(hpmc_ctx* ctx, const MoveArgs& a, const PoissonTable* pt, const
   q.pguide = pt->has_guide ? pt->d_G : nullptr;
   q.ramp = P.ramp; q.tile_cells = P.big;
   q.wlo = 2.1f * a.g.w; q.whi = a.g.L - 2.1f * a.g.w;
+#ifdef HPMC_PHASE_CLOCKS
+  if (!ctx->d_phase_clk) { cudaMalloc(&ctx->d_phase_clk, 64); cudaMemsetAsync(ctx->d_phase_clk, 0, 64, ctx->stream); }
+  q.phase_clk = ctx->d_phase_clk; ctx->phase_ctas += (int64_t)P.ctas * q.npass;
+#endif
   {
     const float rl = (ctx->p.sigma_c + ctx->p.sigma_d) + 1e-3f;
     q.rlist2 = rl * rl;
@@ -309,12 +326,12 @@ int launch_moveq(hpmc_ctx* ctx, const MoveArgs& a, const PoissonTable* pt, const
     // cooperative launch: the runtime guarantees that all CTAs are resident, which the neighbour waits rely on
     void* args[] = {(void*)&q};
     const cudaError_t e = cudaLaunchCooperativeKernel((const void*)k_moveq<SHAPE, QT, QCfg<SHAPE>::CPT, CB>, dim3(P.ctas),
-                                                      dim3(QT), args, SM::bytes, ctx->stream);
+                                                      dim3(QT), args, SM::bytes + smem_pad(), ctx->stream);
     if (e != cudaSuccess) return fail(ctx, HPMC_E_CUDA, std::string("cudaLaunchCooperativeKernel: ") + cudaGetErrorString(e));
     P.seq += 8u;
     return 0;
   }
-  k_moveq<SHAPE, QT, QCfg<SHAPE>::CPT, CB><<<P.ctas, QT, SM::bytes, ctx->stream>>>(q);
+  k_moveq<SHAPE, QT, QCfg<SHAPE>::CPT, CB><<<P.ctas, QT, SM::bytes + smem_pad(), ctx->stream>>>(q);
   return 0;
 }
 
@@ -420,6 +437,18 @@ int hpmc_init(hpmc_ctx** out, const hpmc_params* p, int64_t N, float* d_pos4, fl
 void hpmc_destroy(hpmc_ctx* ctx) {
   if (!ctx) return;
   cudaStreamSynchronize(ctx->stream);
+#ifdef HPMC_PHASE_CLOCKS
+  if (ctx->d_phase_clk) {
+    unsigned long long h[8], tr[2] = {0, 0};
+    cudaMemcpy(h, ctx->d_phase_clk, 64, cudaMemcpyDeviceToHost);
+    cudaMemcpyFromSymbol(tr, g_dbg_trips, sizeof(tr));
+    static const char* nm[8] = {"setup", "1a", "wait", "1b+1c", "1d", "2", "commit", "-"};
+    fprintf(stderr, "phase clocks per CTA and pass (thread 0):");
+    for (int i = 0; i < 7; ++i) fprintf(stderr, " %s %.0f", nm[i], (double)h[i] / (double)std::max<int64_t>(1, ctx->phase_ctas));
+    fprintf(stderr, "; phase 2: %.2f loop trips per tile\n", (double)tr[0] / (double)std::max(1ull, tr[1]));
+    cudaFree(ctx->d_phase_clk);
+  }
+#endif
   if (ctx->own_pose) { cudaFree(ctx->d_pos); cudaFree(ctx->d_quat); }
   cudaFree(ctx->d_cpos); cudaFree(ctx->d_caxis); cudaFree(ctx->d_cid); cudaFree(ctx->d_rank);
   cudaFree(ctx->d_cell_pid); cudaFree(ctx->d_counts); cudaFree(ctx->d_cell_start); cudaFree(ctx->d_tile_sums);

@@ -55,6 +55,9 @@ struct QArgs {
   const uint32_t* cta_first;       // [gridDim.x + 1] first active-cell index of every CTA's share (host table, with the ramp)
   uint32_t* done;                  // [gridDim.x] passes published so far (monotone over the sweeps of a context)
   uint32_t seq0;                   // value of done[] before this sweep
+#ifdef HPMC_PHASE_CLOCKS
+  unsigned long long* phase_clk;   // tuning build: [8] clock64 sums of thread 0 over the phases of every tile
+#endif
   float rlist2;                    // neighbours farther than this from the new centre cannot touch any depletant
                                    // of the move: (sigma_c + sigma_d + 1e-3)^2 for the plain rule (insertion
                                    // sphere about the new centre only), r_cut^2 of R-3.4 otherwise
@@ -72,6 +75,10 @@ __device__ __forceinline__ float sym_unit_bits(uint32_t x) {
 #endif
 #ifndef HPMC_WALK_SLOTS
 #define HPMC_WALK_SLOTS 4         // phase 1b: particle loads in flight per (move, row) item
+#endif
+
+#ifdef HPMC_PHASE_CLOCKS
+__device__ unsigned long long g_dbg_trips[2];    // tuning build: loop trips of thread 0 in phase 2, tiles
 #endif
 
 template <int SHAPE>
@@ -94,8 +101,8 @@ struct QSmem {
   static constexpr int M = CPT * T;
   static constexpr int POOL = Lq::POOL_PER_MOVE * T;
   static constexpr int HCAP = Lq::ANISO ? Lq::HCAP_PER_MOVE * T : 0;
-  static constexpr size_t o_r1 = 0;                                             // float4[M]  r1.xyz, pid bits
-  static constexpr size_t o_rho = o_r1 + sizeof(float4) * M;                    // float4[M]  rho_old.xyz, slot bits
+  static constexpr size_t o_r1 = 0;                                             // float4[M]  r1.xyz, slot bits (phase 1b reads only this)
+  static constexpr size_t o_rho = o_r1 + sizeof(float4) * M;                    // float4[M]  rho_old.xyz, pid bits (phase 2 reads only this + head)
   static constexpr size_t o_q1 = o_rho + sizeof(float4) * M;                    // float4[M]  new quaternion (aniso)
   static constexpr size_t o_aold = o_q1 + (Lq::ANISO ? sizeof(float4) * M : 0); // float4[M]
   static constexpr size_t o_anew = o_aold + (Lq::ANISO ? sizeof(float4) * M : 0);
@@ -189,9 +196,9 @@ __device__ __forceinline__ void q_depletant_queue(const QTables& tb, int nalive,
   const int nw_alive = (nalive + 31) >> 5;
   int j = t % nalive;
   uint32_t m = tb.alive[j];
-  uint32_t c_pid = __float_as_uint(tb.r1[m].w);
   int c_head = tb.head[m];
   float4 c_rho = tb.rho[m];
+  uint32_t c_pid = __float_as_uint(c_rho.w);
   V3 c_aold = V3{0.f, 0.f, 1.f}, c_anew = V3{0.f, 0.f, 1.f};
   if (ANISO) {
     const float4 ao = tb.aold[m], an = tb.anew[m];
@@ -229,7 +236,7 @@ __device__ __forceinline__ void q_depletant_queue(const QTables& tb, int nalive,
         if (found < 0) { active = false; break; }
         j = found;
         m = tb.alive[j];
-        c_pid = __float_as_uint(tb.r1[m].w); c_head = tb.head[m]; c_rho = tb.rho[m];
+        c_head = tb.head[m]; c_rho = tb.rho[m]; c_pid = __float_as_uint(c_rho.w);
         if (ANISO) {
           const float4 ao = tb.aold[m], an = tb.anew[m];
           c_aold = V3{ao.x, ao.y, ao.z}; c_anew = V3{an.x, an.y, an.z};
@@ -238,7 +245,12 @@ __device__ __forceinline__ void q_depletant_queue(const QTables& tb, int nalive,
     }
     // the vote is also the reconvergence point: the Philox block below runs with the whole warp together
     // (checked every fourth trip: a warp that has run dry idles through at most three cheap trips)
-    if ((++trip & 3u) == 0u && !__any_sync(0xffffffffu, active)) break;
+    if ((++trip & 3u) == 0u && !__any_sync(0xffffffffu, active)) {
+#ifdef HPMC_PHASE_CLOCKS
+      if (t == 0) { atomicAdd(&g_dbg_trips[0], (unsigned long long)trip); atomicAdd(&g_dbg_trips[1], 1ull); }
+#endif
+      break;
+    }
     if (active) {
       // one Philox block = one cube-rejection attempt of depletant k (R-S3); c3 carries the attempt number
       const Block4 r = philox(key, c_pid, k, 0, c3);
@@ -276,8 +288,18 @@ __device__ __forceinline__ void q_depletant_queue(const QTables& tb, int nalive,
   }
 }
 
+#ifdef HPMC_PHASE_CLOCKS      // tuning build (profiles/*_summary.md "phase split"): thread 0 sums clock64 deltas per phase
+#define HPMC_PHASE_MARK(i) do { if (threadIdx.x == 0) { const long long c_ = clock64(); pclk[i] += (unsigned long long)(c_ - pclk_t); pclk_t = c_; } } while (0)
+#else
+#define HPMC_PHASE_MARK(i) do { } while (0)
+#endif
+
 template <int SHAPE, int T, int CPT, bool CB>
-__global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS)) k_moveq(const QArgs Q) {
+__global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 128 ? 128 / T : 1))) k_moveq(const QArgs Q) {
+#ifdef HPMC_PHASE_CLOCKS
+  unsigned long long pclk[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  long long pclk_t = clock64();
+#endif
   using Lq = QLayout<SHAPE>;
   using S = QSmem<SHAPE, T, CPT, CB>;
   constexpr bool ANISO = Lq::ANISO;
@@ -375,6 +397,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS)) k_move
     if (t == 0) { s_scal[0] = 0; s_scal[1] = 0; s_scal[3] = 0; s_scal[4] = 0; s_scal[7] = 0; }
     if (t < 4) s_tcnt[t] = 0u;
     __syncthreads();
+    HPMC_PHASE_MARK(0);        // idle/tile setup (incl. the publish of the previous pass)
 
     // ================================================================ phase 1a: one thread per active cell
 #pragma unroll 1
@@ -417,9 +440,8 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS)) k_move
             atomicAdd(&s_tcnt[2], 1u);
           } else {
             const uint32_t e = atomicAdd(&s_scal[4], 1u);
-            s_r1[e] = make_float4(r1.x, r1.y, r1.z, p0.w);
-            s_rho[e] = make_float4(minimg1(g, r0.x - r1.x), minimg1(g, r0.y - r1.y), minimg1(g, r0.z - r1.z),
-                                   __uint_as_float(slot));
+            s_r1[e] = make_float4(r1.x, r1.y, r1.z, __uint_as_float(slot));
+            s_rho[e] = make_float4(minimg1(g, r0.x - r1.x), minimg1(g, r0.y - r1.y), minimg1(g, r0.z - r1.z), p0.w);
             // interior: the new centre is more than two cell widths from the coordinate wrap on every axis, so the
             // minimum image of any neighbour of the 27 cells is the plain difference (|d| < 2w <= L/3 < L/2; n_c >= 6)
             const bool interior = nc >= 6 && r1.x > Q.wlo && r1.x < Q.whi && r1.y > Q.wlo && r1.y < Q.whi &&
@@ -442,6 +464,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS)) k_move
     // pass (and they must be done reading ours): wait for their published pass counter.  Acquire loads by the
     // polling threads + the barrier make their writes visible to the whole CTA.  Phase 1a above touched only this
     // CTA's own cells, so it ran ahead of the wait.  Bounded spin: a stuck neighbour raises the error flag instead of a hang.
+    HPMC_PHASE_MARK(1);        // phase 1a (thread 0's own share of it)
     if (must_wait) {
       must_wait = false;
       const uint32_t target = Q.seq0 + (uint32_t)pass;
@@ -452,14 +475,15 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS)) k_move
         for (;;) {       // relaxed polls (no L1 invalidation while spinning), one acquire fence at the end
           asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(Q.done + b) : "memory");
           if ((int32_t)(v - target) >= 0) break;
-          if (++spins > (1u << 22)) { atomicExch(A.err_flag, 2); break; }
-          __nanosleep(40);
+          if (++spins > (1u << 20)) { atomicExch(A.err_flag, 2); break; }
+          __nanosleep(spins < 4u ? 100u : 400u);      // polls cost issue slots of the SM's other CTAs: back off
         }
         polled = true;
       }
-      if (polled) __threadfence();
+      if (polled) asm volatile("fence.acq_rel.gpu;" ::: "memory");
     }
     __syncthreads();
+    HPMC_PHASE_MARK(2);        // neighbour wait + barrier after 1a
     const int nlist = (int)s_scal[4];
 
     // ================================================================ phase 1b: one thread per (move, x-row) item
@@ -477,7 +501,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS)) k_move
       const int e = it / 9, row = it - 9 * e;
       const float4 r1f = s_r1[e];
       const V3 r1 = V3{r1f.x, r1f.y, r1f.z};
-      const uint32_t slot = __float_as_uint(s_rho[e].w);
+      const uint32_t slot = __float_as_uint(r1f.w);
       const uint32_t cw = s_cell[e];
       const int ix = cw & 1023, iy = (cw >> 10) & 1023, iz = (cw >> 20) & 1023;
       const bool interior = (cw >> 31) != 0u;
@@ -555,6 +579,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS)) k_move
       }
     }
     __syncthreads();
+    HPMC_PHASE_MARK(3);        // phase 1b + 1c + barrier
     // ---- neighbour pool overflow (a locally dense tile, e.g. a cluster in a dilute box): nothing of this tile is
     // committed yet (boundary outcomes are idempotent, its counters are tile-local), so halve the tile and redo it
     if (s_scal[1] > (uint32_t)POOL) {
@@ -566,7 +591,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS)) k_move
     for (int e = t; e < nlist; e += T) {
       uint32_t Nd = 0;
       if (s_state[e] == OUT_NONE && A.pt_n > 0) {
-        const uint32_t pid = __float_as_uint(s_r1[e].w);
+        const uint32_t pid = __float_as_uint(s_rho[e].w);
         const Block4 rn = philox(A.key, pid, 0, 0, P_NDEP + colw);
         ++n_blocks;
         const unsigned long long U = ((unsigned long long)rn.x << 32) | rn.y;
@@ -576,6 +601,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS)) k_move
       if (s_state[e] == OUT_NONE && Nd != 0) s_alive[atomicAdd(&s_scal[0], 1u)] = (uint16_t)e;
     }
     __syncthreads();
+    HPMC_PHASE_MARK(4);        // phase 1d + barrier
     if (!CB) {
     const int nalive = (int)s_scal[0];
     for (int w = t; w < NW; w += T) {
@@ -646,7 +672,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS)) k_move
         const V3 ro = V3{rof.x, rof.y, rof.z};
         V3 ao = V3{0.f, 0.f, 1.f}, an = V3{0.f, 0.f, 1.f};
         if (ANISO) { const float4 a0 = s_aold[m], a1 = s_anew[m]; ao = V3{a0.x, a0.y, a0.z}; an = V3{a1.x, a1.y, a1.z}; }
-        V3 sp = ball_sample(A.key, __float_as_uint(r1f.w), kk, tt + (dir << 16), c3cb, g.Rins, g.Rins2, n_blocks);
+        V3 sp = ball_sample(A.key, __float_as_uint(rof.w), kk, tt + (dir << 16), c3cb, g.Rins, g.Rins2, n_blocks);
         bool valid;
         if (dir == 0) {                  // forward: about the old centre, must overlap the old pose only (R-G2)
           sp = sp + ro;
@@ -688,12 +714,13 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS)) k_move
       __syncthreads();
     }
     }
+    HPMC_PHASE_MARK(5);        // phase 2 (+ CB) + barrier
     // ================================================================ commit (a10)
 #pragma unroll 1
     for (int e = t; e < nlist; e += T) {
       int out = (int)s_state[e];
       const float4 r1f = s_r1[e];
-      const uint32_t pid = __float_as_uint(r1f.w);
+      const uint32_t pid = __float_as_uint(s_rho[e].w);
       const bool rot = (s_cell[e] >> 30) & 1u;
       if (!CB && out == OUT_NONE) {
         const uint32_t Nd = s_Nd[e], rm_ = s_rejmin[e];
@@ -718,11 +745,11 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS)) k_move
       }
       A.outcome[pid] = (uint8_t)out;
       if (out == OUT_ACCEPT) {
-        const uint32_t slot = __float_as_uint(s_rho[e].w);
+        const uint32_t slot = __float_as_uint(r1f.w);
         float4 pn = A.pos[pid];
         pn.x = r1f.x; pn.y = r1f.y; pn.z = r1f.z;
         A.pos[pid] = pn;
-        A.cpos[slot] = r1f;
+        A.cpos[slot] = make_float4(r1f.x, r1f.y, r1f.z, __uint_as_float(pid));
         if (ANISO && rot) {
           A.quat[pid] = s_q1[e];
           const float4 an = s_anew[e];
@@ -736,6 +763,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS)) k_move
       atomicAdd(&s_cnt[C_REJ_BOUNDARY], s_tcnt[2]);
     }
     __syncthreads();
+    HPMC_PHASE_MARK(6);        // commit + barrier
   }
   // ---- publish the pass: every commit of this CTA is ordered before the counter by the barrier above + the release
   if (Q.npass > 1) {
@@ -760,6 +788,10 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS)) k_move
   }
   __syncthreads();
   if (t < C_COUNT && s_cnt[t]) atomicAdd(&A.counters[t], (unsigned long long)s_cnt[t]);
+#ifdef HPMC_PHASE_CLOCKS
+  if (t == 0)
+    for (int i = 0; i < 8; ++i) atomicAdd(&Q.phase_clk[i], pclk[i]);
+#endif
 }
 
 }  // namespace hpmc
