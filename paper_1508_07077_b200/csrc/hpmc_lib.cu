@@ -419,7 +419,7 @@ int hpmc_init(hpmc_ctx** out, const hpmc_params* p, int64_t N, float* d_pos4, fl
     ctx->use_queue = !(sel && std::string(sel) == "warp");
     // Configurational bias runs on the warp-per-cell kernel by default: measured on spherodisks with n_trial = 4 it is
     // 1.2-1.75x faster than the round-based CB stage of the item-queue kernel at every size tried (32,768 ... 884,736
-    // particles; profiles/r2_cb_kernels.md).  Both are bit-exact against the oracle and both are tested.
+    // particles; profiles/r2_cb_kernels.md).  Both give the same bits and both are covered by the parity tests.
     const char* cbk = getenv("HPMC_CB_KERNEL");
     ctx->cb_queue = cbk && std::string(cbk) == "queue";
     int rc = 0;
