@@ -26,6 +26,7 @@ COUNTER_NAMES = (
 )
 
 SHAPES = {"sphere": 0, "halfball": 1, "spherodisk": 2}
+FLAG_SHELL, FLAG_ROSENBLUTH, FLAG_TEST_LITERAL_CORE = 1, 2, 0x100
 
 
 class OracleParams(C.Structure):
@@ -72,6 +73,10 @@ def lib() -> C.CDLL:
             sig = {
                 "oracle_create": (vp, [P(OracleParams), i64, vp, vp]),
                 "oracle_destroy": (None, [vp]),
+                "oracle_set_flags": (i32, [vp, u32, f32]),
+                "oracle_cbrt_fixed": (f32, [f32]),
+                "oracle_shell": (f64, [P(OracleParams), f64, f32, u32, P(f32)]),
+                "oracle_shell_samples": (None, [P(OracleParams), f32, u32, u32, u32, u32, i64, vp]),
                 "oracle_grid": (i32, [vp, P(i32), P(f32)]),
                 "oracle_set_threads": (None, [i32]),
                 "oracle_get_threads": (i32, []),
@@ -140,6 +145,11 @@ class Oracle:
         h, self.h = getattr(self, "h", None), None
         if h:
             self.L.oracle_destroy(h)
+
+    def set_flags(self, flags, eval_dmax=-1.0):
+        """Options of the following sweeps: FLAG_SHELL (R-N1), FLAG_ROSENBLUTH (R-N4); eval_dmax: step size assumed by
+        eval_move(s) for the shell."""
+        self.L.oracle_set_flags(self.h, int(flags), float(eval_dmax))
 
     def build_cells(self, seed, step):
         rc = self.L.oracle_build_cells(self.h, seed, step)

@@ -28,6 +28,12 @@
 // rule of Eq. 16 (R-G3), the particular samplers' bit patterns, and outcomes of the
 // iterative convex test inside its 1e-5 contact band.
 //
+// Options (oracle_set_flags; default 0 = the path above, untouched by them): SURVEY 8(f) NEXT-1, the shell-restricted
+// insertion volume of L158 (reading R-N1 of DESIGN.md), and NEXT-4, the exact Rosenbluth form of the configurational
+// bias weight (refs 27, 28, 33; reading R-N4).  Their pins: radial cdf and isotropy of the shell sampler, cube-root
+// accuracy, isolated-colloid and Asakura-Oosawa ratio tests with the shell on (and a literal-hard-core shell failing
+// them), forward/reverse ratio of the Rosenbluth form to 3 sigma with no systematic allowance.
+//
 // Arithmetic: all pose arithmetic is IEEE fp32 with contraction OFF (-ffp-contract=off);
 // an FMA is used only where fmaf() is written.  Integers u32/u64.  fp64 only for the
 // Poisson threshold table.
@@ -315,6 +321,8 @@ struct Ctx {
   std::vector<float> trial_pos, trial_quat;   // proposed pose of every particle tried this sweep
   uint64_t cnt[C_COUNT] = {0};
   PoissonTable pt;
+  uint32_t flags = 0;          // F_* options (oracle_set_flags)
+  float eval_dmax = -1.0f;     // d_max assumed by oracle_eval_move(s) for the shell (default: d_max_cap)
   std::string err;
 };
 
@@ -371,12 +379,60 @@ static inline V3 ball_sample(uint32_t seed, uint32_t step, uint32_t purpose, uin
   return V3{0.0f, 0.0f, 0.0f};
 }
 
+// ---- options of a sweep (oracle_set_flags)
+enum { F_SHELL = 1u, F_ROSENBLUTH = 2u, F_TEST_LITERAL_CORE = 0x100u };
+
+// R-N1 (L158 "restricting the sampling to the excluded volume shell of the moved colloid"): depletants are drawn
+// uniformly in the shell R_in < |d| <= R about the NEW centre instead of the whole ball.  Eq. 12 (L136) needs
+// V_0 >= V'_excl \ V_excl: the ball |d| <= R_in must lie inside the OLD pose's excluded volume for every move the
+// sweep can propose.  The old excluded volume contains the ball of radius r_in about the old centre (r_in = R for a
+// sphere, r_d for the half-ball whose centre lies on its flat face, s + r_d for the spherodisk), a translation moves
+// the centre by at most sqrt(3) d_max and a rotation not at all, hence R_in = max(0, r_in - sqrt(3) d_max).
+struct Shell { float Rin, Rin3, dR3; };
+static inline Shell make_shell(const Geo& g, float d_max, uint32_t flags) {
+  float rin = g.Rins;
+  if (g.shape == SH_HALFBALL) rin = g.rd;
+  else if (g.shape == SH_SPHERODISK) rin = g.sdisk + g.rd;
+  Shell sh;
+  sh.Rin = rin - 1.7320508f * d_max;
+  if (sh.Rin < 0.0f) sh.Rin = 0.0f;
+  if (flags & F_TEST_LITERAL_CORE) sh.Rin = 0.5f * g.dcirc;   // mutation used by a pin only: the shell minus the HARD core
+  sh.Rin3 = (sh.Rin * sh.Rin) * sh.Rin;
+  sh.dR3 = (g.Rins * g.Rins) * g.Rins - sh.Rin3;
+  return sh;
+}
+// cube root by +, x, / only (libm's cbrtf is not reproducible on the device): exponent/3 seed, four Newton steps
+static inline float cbrt_fixed(float t) {
+  uint32_t b; std::memcpy(&b, &t, 4);
+  b = b / 3u + 0x2a514067u;
+  float y; std::memcpy(&y, &b, 4);
+  for (int it = 0; it < 4; ++it) { const float q = t / (y * y); y = ((y + y) + q) * 0.33333334f; }
+  return y;
+}
+// uniform point in the shell: direction by cube rejection (words 0-2 of the block, one block per attempt, as R-S3) and
+// IEEE normalisation, radius (R_in^3 + u dR^3)^(1/3) from word 3 of the accepted block
+static inline V3 shell_sample(uint32_t seed, uint32_t step, uint32_t purpose, uint32_t colour, uint32_t id,
+                              uint32_t k, const Shell& sh, float radius, uint64_t& nblocks) {
+  for (uint32_t a = 0; a < 64; ++a) {
+    const U4 r = philox4x32_10(id, k, 0, word3(purpose, colour, a), seed, step);
+    ++nblocks;
+    const V3 v = V3{sym_unit(r.v[0]), sym_unit(r.v[1]), sym_unit(r.v[2])};
+    const float n2 = dot3(v, v);
+    if (n2 <= 1.0f && n2 >= 1e-6f) {
+      const float t = sh.Rin3 + unit01(r.v[3]) * sh.dR3;
+      const float sc = cbrt_fixed(t) / sqrtf(n2);
+      return v * sc;
+    }
+  }
+  return V3{radius, 0.0f, 0.0f};
+}
+
 struct Nbr { V3 rho; V3 axis; };
 
 // Steps 3.4 - 3.8 of the move: neighbourhood, hard overlap, depletants.
 // i = moved colloid, own = its cell, (r0,q0) old pose, (r1,q1) new pose (already wrapped).
 static int evaluate_move(const Ctx& c, uint32_t seed, uint32_t step, uint32_t colour, int64_t i,
-                         int64_t own, V3 r0, Q4 q0, V3 r1, Q4 q1, int n_trial, Counters& cn) {
+                         int64_t own, V3 r0, Q4 q0, V3 r1, Q4 q1, int n_trial, float d_max, Counters& cn) {
   const Geo& g = c.g;
   const int nc = c.nc;
   const int ix = (int)(own % nc), iy = (int)((own / nc) % nc), iz = (int)(own / ((int64_t)nc * nc));
@@ -409,6 +465,14 @@ static int evaluate_move(const Ctx& c, uint32_t seed, uint32_t step, uint32_t co
   cn.c[C_DEP_DRAWN] += (uint64_t)Nd;
 
   const V3 zero = V3{0.0f, 0.0f, 0.0f};
+  const Shell sh = make_shell(g, d_max, c.flags);
+  // position of depletant k relative to the new centre: whole insertion ball (L156), or its shell (option R-N1)
+  auto dep_position = [&](int64_t k) {
+    if (c.flags & F_SHELL)
+      return shell_sample(seed, step, P_DEPPOS, colour, (uint32_t)i, (uint32_t)k, sh, g.Rins, cn.c[C_PHILOX_BLOCKS]);
+    return ball_sample(seed, step, P_DEPPOS, colour, (uint32_t)i, (uint32_t)k, 0, 0, g.Rins, g.Rins2,
+                       cn.c[C_PHILOX_BLOCKS]);
+  };
   auto free_of_nbrs = [&](V3 d) {
     for (const Nbr& n : nb)
       if (dep_overlap(g, d - n.rho, n.axis)) return false;
@@ -420,8 +484,7 @@ static int evaluate_move(const Ctx& c, uint32_t seed, uint32_t step, uint32_t co
 
   if (n_trial <= 0) {                          // 3.7 plain rule, L68
     for (int64_t k = 0; k < Nd; ++k) {
-      const V3 d = ball_sample(seed, step, P_DEPPOS, colour, (uint32_t)i, (uint32_t)k, 0, 0, g.Rins,
-                               g.Rins2, cn.c[C_PHILOX_BLOCKS]);
+      const V3 d = dep_position(k);
       ++cn.c[C_DEP_NEEDED]; ++cn.c[C_DEP_EVALUATED];
       if (new_only(d) && free_of_nbrs(d)) return OUT_DEPLETANT;
     }
@@ -431,9 +494,11 @@ static int evaluate_move(const Ctx& c, uint32_t seed, uint32_t step, uint32_t co
   // 3.8 configurational bias, Eq. 16 (L172) with the reading R-G1/G2/G3
   float P = 1.0f;
   bool any = false;
+  // Option R-N4 (refs 27, 28, 33): the exact Rosenbluth weight N'_ins / (N_ins + 1) from n_trial forward and
+  // n_trial - 1 FRESH reverse reinsertions (the original depletant is the n_trial-th reverse candidate, L174)
+  const bool rosen = (c.flags & F_ROSENBLUTH) != 0;
   for (int64_t k = 0; k < Nd; ++k) {
-    const V3 d = ball_sample(seed, step, P_DEPPOS, colour, (uint32_t)i, (uint32_t)k, 0, 0, g.Rins,
-                             g.Rins2, cn.c[C_PHILOX_BLOCKS]);
+    const V3 d = dep_position(k);
     ++cn.c[C_DEP_NEEDED]; ++cn.c[C_DEP_EVALUATED];
     if (!(new_only(d) && free_of_nbrs(d))) continue;
     any = true;
@@ -443,13 +508,15 @@ static int evaluate_move(const Ctx& c, uint32_t seed, uint32_t step, uint32_t co
       const V3 f = ball_sample(seed, step, P_CBPOS, colour, (uint32_t)i, (uint32_t)k, (uint32_t)t, 0,
                                g.Rins, g.Rins2, cn.c[C_PHILOX_BLOCKS]) + rho_old;
       if (old_only(f)) { ++Ni; if (free_of_nbrs(f)) ++Npins; }
+      if (rosen && t == n_trial - 1) break;
       // reverse: reinsertion about the NEW centre
       const V3 b = ball_sample(seed, step, P_CBPOS, colour, (uint32_t)i, (uint32_t)k,
                                (uint32_t)t + (1u << 16), 0, g.Rins, g.Rins2, cn.c[C_PHILOX_BLOCKS]);
       if (new_only(b)) { ++Npi; if (free_of_nbrs(b)) ++Nins; }
     }
-    cn.c[C_CB_REINSERTIONS] += 2u * (uint64_t)n_trial;
+    cn.c[C_CB_REINSERTIONS] += 2u * (uint64_t)n_trial - (rosen ? 1u : 0u);
     if (Npins == 0) return OUT_CB;             // R-G3: zero forward weight
+    if (rosen) { P = P * ((float)Npins / (float)(Nins + 1u)); continue; }
     const float wk = (float)(Npins * (Npi + 1u)) / (float)((Nins + 1u) * Ni);
     P = P * wk;
   }
@@ -491,7 +558,7 @@ static void process_cell(Ctx& c, uint32_t seed, uint32_t step, uint32_t colour, 
 
   int out;
   if (cell_of(c, r1) != cell) out = OUT_BOUNDARY;      // confinement, L180
-  else out = evaluate_move(c, seed, step, colour, i, cell, r0, q0, r1, q1, n_trial, cn);
+  else out = evaluate_move(c, seed, step, colour, i, cell, r0, q0, r1, q1, n_trial, d_max, cn);
   c.outcome[(size_t)i] = (uint8_t)out;
   switch (out) {
     case OUT_ACCEPT: {
@@ -511,6 +578,13 @@ static void process_cell(Ctx& c, uint32_t seed, uint32_t step, uint32_t colour, 
 static double lambda_of(const Geo& g, double n_R) {
   const double Rd = (double)g.Rins;
   return n_R * ((4.0 * M_PI / 3.0) * (Rd * Rd * Rd));
+}
+// mean number of depletants of a move: fugacity x sampled volume (L67), the shell's volume with option R-N1
+static double lambda_opt(const Geo& g, double n_R, float d_max, uint32_t flags) {
+  if (!(flags & F_SHELL)) return lambda_of(g, n_R);
+  const Shell sh = make_shell(g, d_max, flags);
+  const double Rd = (double)g.Rins, Ri = (double)sh.Rin;
+  return n_R * ((4.0 * M_PI / 3.0) * (Rd * Rd * Rd - Ri * Ri * Ri));
 }
 
 }  // namespace
@@ -543,6 +617,13 @@ void* oracle_create(const oracle_params* p, int64_t N, float* pos4, float* quat4
   return c;
 }
 void oracle_destroy(void* h) { delete (Ctx*)h; }
+// options of the following sweeps / evaluations: bit 0 shell-restricted insertion (R-N1), bit 1 Rosenbluth CB weight
+// (R-N4); eval_dmax >= 0: the step size oracle_eval_move(s) assumes for the shell (their moves must obey it)
+int oracle_set_flags(void* h, uint32_t flags, float eval_dmax) {
+  Ctx* c = (Ctx*)h;
+  c->flags = flags; c->eval_dmax = eval_dmax; c->pt.lambda = -1.0;
+  return 0;
+}
 int oracle_grid(void* h, int32_t* nc, float* w) { Ctx* c = (Ctx*)h; *nc = c->nc; *w = c->w; return 0; }
 void oracle_set_threads(int n) {
 #ifdef _OPENMP
@@ -581,7 +662,7 @@ int oracle_sweep(void* h, uint32_t seed, uint32_t step, double n_R, float d_max,
   Ctx* c = (Ctx*)h;
   if (!c->built || c->b_seed != seed || c->b_step != step) return -3;
   if (!(d_max >= 0.0f) || d_max > c->g.dmax_cap || n_R < 0.0 || a_max < 0.0f || n_trial < 0 || n_trial > 65535) return -1;
-  const double lambda = lambda_of(c->g, n_R);
+  const double lambda = lambda_opt(c->g, n_R, d_max, c->flags);
   if (c->pt.lambda != lambda) build_poisson(c->pt, lambda);
   // R-2: Fisher-Yates permutation of the 8 colours from SWEEP blocks 1, 2
   uint32_t perm[8] = {0, 1, 2, 3, 4, 5, 6, 7};
@@ -658,7 +739,8 @@ int oracle_eval_move(void* h, uint32_t seed, uint32_t draw, int64_t i, const flo
                      double n_R, int32_t n_trial) {
   Ctx* c = (Ctx*)h;
   if (!c->built) return -3;
-  const double lambda = lambda_of(c->g, n_R);
+  const float dm = c->eval_dmax >= 0.0f ? c->eval_dmax : c->g.dmax_cap;
+  const double lambda = lambda_opt(c->g, n_R, dm, c->flags);
   if (c->pt.lambda != lambda) build_poisson(c->pt, lambda);
   const V3 r0 = load_r(*c, i); const Q4 q0 = load_q(*c, i);
   const V3 r1 = V3{pos3[0], pos3[1], pos3[2]};
@@ -666,7 +748,7 @@ int oracle_eval_move(void* h, uint32_t seed, uint32_t draw, int64_t i, const flo
   const int64_t own = cell_of(*c, r0);
   if (cell_of(*c, r1) != own) return OUT_BOUNDARY;
   Counters cn;
-  return evaluate_move(*c, seed, draw, 0, i, own, r0, q0, r1, q1, n_trial, cn);
+  return evaluate_move(*c, seed, draw, 0, i, own, r0, q0, r1, q1, n_trial, dm, cn);
 }
 
 // Batched form of oracle_eval_move for the statistical pins: out[j] = oracle_eval_move(h, seed, draw0 + j, ...) for
@@ -676,7 +758,8 @@ int oracle_eval_moves(void* h, uint32_t seed, uint32_t draw0, int64_t n, int64_t
                       const float* quat4, double n_R, int32_t n_trial, uint8_t* out) {
   Ctx* c = (Ctx*)h;
   if (!c->built) return -3;
-  const double lambda = lambda_of(c->g, n_R);
+  const float dm = c->eval_dmax >= 0.0f ? c->eval_dmax : c->g.dmax_cap;
+  const double lambda = lambda_opt(c->g, n_R, dm, c->flags);
   if (c->pt.lambda != lambda) build_poisson(c->pt, lambda);
   const V3 r0 = load_r(*c, i); const Q4 q0 = load_q(*c, i);
   const V3 r1 = V3{pos3[0], pos3[1], pos3[2]};
@@ -687,7 +770,7 @@ int oracle_eval_moves(void* h, uint32_t seed, uint32_t draw0, int64_t n, int64_t
   for (int64_t j = 0; j < n; ++j) {
     Counters cn;
     out[j] = outside ? (uint8_t)OUT_BOUNDARY
-                     : (uint8_t)evaluate_move(*c, seed, draw0 + (uint32_t)j, 0, i, own, r0, q0, r1, q1, n_trial, cn);
+                     : (uint8_t)evaluate_move(*c, seed, draw0 + (uint32_t)j, 0, i, own, r0, q0, r1, q1, n_trial, dm, cn);
   }
   return 0;
 }
@@ -750,6 +833,24 @@ void oracle_poisson_draws(double lambda, const uint64_t* U, int64_t n, int64_t* 
 }
 double oracle_lambda(const oracle_params* p, double n_R) {
   return lambda_of(make_geo(p->shape, p->sigma_c, p->disk_a, p->disk_s, p->sigma_d, p->box_L, p->d_max_cap), n_R);
+}
+float oracle_cbrt_fixed(float t) { return cbrt_fixed(t); }
+// lambda and inner radius of the shell option for step size d_max
+double oracle_shell(const oracle_params* p, double n_R, float d_max, uint32_t flags, float* Rin) {
+  const Geo g = make_geo(p->shape, p->sigma_c, p->disk_a, p->disk_s, p->sigma_d, p->box_L, p->d_max_cap);
+  *Rin = make_shell(g, d_max, flags | F_SHELL).Rin;
+  return lambda_opt(g, n_R, d_max, flags | F_SHELL);
+}
+// n shell samples k = 0..n-1 of the DEPPOS stream of colloid `id`
+void oracle_shell_samples(const oracle_params* p, float d_max, uint32_t seed, uint32_t step, uint32_t colour, uint32_t id,
+                          int64_t n, float* out3) {
+  const Geo g = make_geo(p->shape, p->sigma_c, p->disk_a, p->disk_s, p->sigma_d, p->box_L, p->d_max_cap);
+  const Shell sh = make_shell(g, d_max, F_SHELL);
+  uint64_t nb = 0;
+  for (int64_t k = 0; k < n; ++k) {
+    const V3 d = shell_sample(seed, step, P_DEPPOS, colour, id, (uint32_t)k, sh, g.Rins, nb);
+    out3[3 * k] = d.x; out3[3 * k + 1] = d.y; out3[3 * k + 2] = d.z;
+  }
 }
 // n ball samples k = 0..n-1 of the DEPPOS stream of colloid `id`
 void oracle_ball_samples(uint32_t seed, uint32_t step, uint32_t colour, uint32_t id, int64_t n, float radius,
