@@ -73,7 +73,7 @@ typedef struct {
   uint64_t dep_needed;      /* sum of (index of the first rejecting depletant + 1), or N_d if none: the
                                sequential algorithm's work; identical in the oracle */
   uint64_t dep_evaluated;   /* depletant positions the kernel actually generated (>= dep_needed) */
-  uint64_t cb_reinsertions; /* 2 n_trial per rejecting depletant handled (Sec. III.D) */
+  uint64_t cb_reinsertions; /* 2 n_trial per rejecting depletant handled (Sec. III.D); 2 n_trial - 1 with HPMC_OPT_ROSENBLUTH */
   uint64_t philox_blocks;   /* Philox4x32-10 blocks computed (warp-uniform ones counted once) */
 } hpmc_counters_t;
 
@@ -107,6 +107,21 @@ int hpmc_build_cells(hpmc_ctx* ctx, uint32_t seed, uint32_t step);
  * Requires hpmc_build_cells(seed, step) before it, else HPMC_E_STATE; d_max <= d_max_cap else HPMC_E_DMAX.
  * Asynchronous; poses are updated in place. */
 int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_max, float a_max, int32_t n_trial);
+
+/* Options of the sweeps that follow (persistent; default 0 = the path exactly as described above).
+ *   HPMC_OPT_SHELL       SURVEY 8(f) NEXT-1, PAPER.md L158 ("restricting the sampling to the excluded volume shell of
+ *                        the moved colloid"), reading R-N1: depletants are drawn uniformly in the shell
+ *                        R_in < |d| <= R about the new centre, R = (sigma_c + sigma_d)/2, R_in = max(0, r_in - sqrt(3) d_max)
+ *                        with r_in = R (sphere), sigma_d/2 (half-ball), disk_s + sigma_d/2 (spherodisk): the largest
+ *                        concentric ball that lies inside the OLD pose's excluded volume for every move of the sweep,
+ *                        which is what Eq. 12 (L136) requires.  N_d ~ Poisson(n_R V_shell).  Same transition rate
+ *                        (Eq. 15), fewer insertions: the shell is 42 % of the ball at C3's d_max = 0.05.
+ *   HPMC_OPT_ROSENBLUTH  NEXT-4, refs 27, 28, 33 (L288-294), reading R-N4: with n_trial > 0 the weight of a rejecting
+ *                        depletant is N'_ins / (N_ins + 1) from n_trial forward and n_trial - 1 fresh reverse
+ *                        reinsertions (the exact Rosenbluth form) instead of Eq. 16 as printed / adopted (R-G1).
+ * Unknown bits: HPMC_E_BADARG.  Host-side only, takes effect with the next hpmc_sweep. */
+enum { HPMC_OPT_SHELL = 1, HPMC_OPT_ROSENBLUTH = 2 };
+int hpmc_set_options(hpmc_ctx* ctx, uint32_t options);
 
 /* n_sweeps x (hpmc_build_cells + hpmc_sweep) with step = step0, step0+1, ...  Asynchronous. */
 int hpmc_run(hpmc_ctx* ctx, uint32_t seed, uint32_t step0, int64_t n_sweeps, double n_R, float d_max, float a_max,

@@ -77,6 +77,7 @@ struct hpmc_ctx {
   int num_sms = 148;
   int move_ctas = 0;
   QPlan plan[2];                       // launch plans of the item-queue move kernel: [0] plain rule, [1] configurational bias
+  uint32_t options = 0;                // hpmc_set_options
   bool use_queue = true;               // HPMC_MOVE_KERNEL=warp selects the first (warp-per-cell) design
   bool cb_queue = false;               // HPMC_CB_KERNEL=queue: configurational bias through the item-queue kernel too
   int64_t launches = 0;
@@ -501,7 +502,18 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
   if (!ctx->built || ctx->b_seed != seed || ctx->b_step != step)
     return fail(ctx, HPMC_E_STATE, "hpmc_sweep: call hpmc_build_cells(seed, step) first");
   const double Rd = (double)ctx->g.Rins;
-  const double lambda = n_R * ((4.0 * M_PI / 3.0) * (Rd * Rd * Rd));
+  double lambda = n_R * ((4.0 * M_PI / 3.0) * (Rd * Rd * Rd));
+  // HPMC_OPT_SHELL (R-N1, L158): R_in = max(0, r_in - sqrt(3) d_max), r_in = inradius of the dilated shape about its centre
+  float sh_Rin = 0.0f;
+  if (ctx->options & HPMC_OPT_SHELL) {
+    float rin = ctx->g.Rins;
+    if (ctx->p.shape == HPMC_HALFBALL) rin = ctx->g.rd;
+    else if (ctx->p.shape == HPMC_SPHERODISK) rin = ctx->g.sdisk + ctx->g.rd;
+    sh_Rin = rin - 1.7320508f * d_max;
+    if (sh_Rin < 0.0f) sh_Rin = 0.0f;
+    const double Ri = (double)sh_Rin;
+    lambda = n_R * ((4.0 * M_PI / 3.0) * (Rd * Rd * Rd - Ri * Ri * Ri));
+  }
   PoissonTable* pt = nullptr;
   const int rc = get_table(ctx, lambda, &pt);
   if (rc) return rc;
@@ -526,6 +538,9 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
   a.cell_start = ctx->d_cell_start;
   a.ptable = pt->d_T; a.pt_n = pt->n; a.pt_klo = pt->k_lo;
   a.outcome = ctx->d_outcome; a.counters = ctx->d_counters; a.err_flag = ctx->d_err;
+  a.options = ctx->options;
+  a.sh_Rin3 = (sh_Rin * sh_Rin) * sh_Rin;
+  a.sh_dR3 = (ctx->g.Rins * ctx->g.Rins) * ctx->g.Rins - a.sh_Rin3;
   const bool cb = n_trial > 0;
   // timing: ONE event pair around the 8 launches of the sweep (an event pair per launch costs more than the gaps
   // between the launches it would exclude); hpmc_move_kernel_ms counts 8 launches per pair
@@ -571,6 +586,13 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
   ctx->launches += nlaunch;
   CU(cudaGetLastError());
   ctx->built = false;
+  return HPMC_OK;
+}
+
+int hpmc_set_options(hpmc_ctx* ctx, uint32_t options) {
+  if (!ctx) return HPMC_E_BADARG;
+  if (options & ~(uint32_t)(HPMC_OPT_SHELL | HPMC_OPT_ROSENBLUTH)) return fail(ctx, HPMC_E_BADARG, "hpmc_set_options: unknown option bit");
+  ctx->options = options;
   return HPMC_OK;
 }
 

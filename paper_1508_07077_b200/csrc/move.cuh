@@ -46,7 +46,31 @@ struct MoveArgs {
   uint8_t* outcome;
   unsigned long long* counters;
   int* err_flag;
+  uint32_t options;                    // OPT_SHELL | OPT_ROSENBLUTH (hpmc_set_options)
+  float sh_Rin3, sh_dR3;               // shell option (R-N1): R_in^3 and R^3 - R_in^3
 };
+
+enum : uint32_t { OPT_SHELL = 1u, OPT_ROSENBLUTH = 2u };
+
+// cube root by +, x, / only (R-N1: no libdevice transcendental on the parity path): exponent/3 seed, four Newton steps
+__device__ __forceinline__ float cbrt_fixed(float t) {
+  float y = __uint_as_float(__float_as_uint(t) / 3u + 0x2a514067u);
+#pragma unroll
+  for (int it = 0; it < 4; ++it) { const float q = __fdiv_rn(t, y * y); y = ((y + y) + q) * 0.33333334f; }
+  return y;
+}
+
+// One attempt of the shell sampler (R-N1) from one Philox block: direction by cube rejection (words 0-2), radius
+// (R_in^3 + u dR^3)^(1/3) from word 3.  Returns false if the attempt is rejected.
+__device__ __forceinline__ bool shell_attempt(const Block4& r, float Rin3, float dR3, V3& d) {
+  const V3 v = V3{sym_unit(r.x), sym_unit(r.y), sym_unit(r.z)};
+  const float n2 = dot3(v, v);
+  if (!(n2 <= 1.0f && n2 >= 1e-6f)) return false;
+  const float t = Rin3 + unit01(r.w) * dR3;
+  d = v * __fdiv_rn(cbrt_fixed(t), __fsqrt_rn(n2));
+  return true;
+}
+
 
 // uniform point in the ball (R-S3): cube rejection, one Philox block per attempt, cap 64 then the origin
 __device__ __forceinline__ V3 ball_sample(const Key10& key, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3base,
@@ -58,6 +82,18 @@ __device__ __forceinline__ V3 ball_sample(const Key10& key, uint32_t c0, uint32_
     if (dot3(d, d) <= radius2) return d;
   }
   return V3{0.0f, 0.0f, 0.0f};
+}
+
+// position of depletant k about the new centre: the whole insertion ball (L156) or, with OPT_SHELL, its shell (L158)
+__device__ __forceinline__ V3 dep_position(const MoveArgs& A, uint32_t pid, uint32_t k, uint32_t c3dep, uint32_t& nblocks) {
+  if (!(A.options & OPT_SHELL)) return ball_sample(A.key, pid, k, 0, c3dep, A.g.Rins, A.g.Rins2, nblocks);
+  for (uint32_t a = 0; a < 64; ++a) {
+    const Block4 r = philox(A.key, pid, k, 0, c3dep + (a << 16));
+    ++nblocks;
+    V3 d;
+    if (shell_attempt(r, A.sh_Rin3, A.sh_dR3, d)) return d;
+  }
+  return V3{A.g.Rins, 0.0f, 0.0f};
 }
 
 template <int SHAPE>
@@ -244,7 +280,7 @@ __global__ void __launch_bounds__(MOVE_WARPS * 32) k_move(const MoveArgs A) {
             const uint32_t k = base + lane;
             bool rej = false;
             if (k < Nd) {
-              const V3 d = ball_sample(A.key, pid, k, 0, c3dep, g.Rins, g.Rins2, lane_blocks);
+              const V3 d = dep_position(A, pid, k, c3dep, lane_blocks);
               ++lane_eval;
               rej = new_only<SHAPE>(g, m, d) && free_of_nbrs<SHAPE>(g, m, d);
             }
@@ -257,11 +293,14 @@ __global__ void __launch_bounds__(MOVE_WARPS * 32) k_move(const MoveArgs A) {
           float P = 1.0f;
           bool any = false, zero = false;
           const uint32_t ne = 2u * (uint32_t)A.n_trial;
+          // OPT_ROSENBLUTH (R-N4): the last reverse reinsertion is not drawn (the original depletant takes its place)
+          const bool rosen = (A.options & OPT_ROSENBLUTH) != 0u;
+          const uint32_t e_skip = rosen ? ne - 1u : 0xffffffffu;
           for (uint32_t base = 0; base < Nd && !zero; base += 32) {
             const uint32_t k = base + lane;
             bool rej = false;
             if (k < Nd) {
-              const V3 d = ball_sample(A.key, pid, k, 0, c3dep, g.Rins, g.Rins2, lane_blocks);
+              const V3 d = dep_position(A, pid, k, c3dep, lane_blocks);
               ++lane_eval;
               rej = new_only<SHAPE>(g, m, d) && free_of_nbrs<SHAPE>(g, m, d);
             }
@@ -275,7 +314,7 @@ __global__ void __launch_bounds__(MOVE_WARPS * 32) k_move(const MoveArgs A) {
                 const uint32_t e = e0 + lane;
                 bool valid = false, fr = false;
                 const uint32_t dir = e & 1u, t = e >> 1;
-                if (e < ne) {
+                if (e < ne && e != e_skip) {
                   V3 s = ball_sample(A.key, pid, kk, t + (dir << 16), c3cb, g.Rins, g.Rins2, lane_blocks);
                   if (dir == 0) {                 // forward: about the old centre, must overlap the old pose only
                     s = s + m.rho_old;
@@ -289,9 +328,10 @@ __global__ void __launch_bounds__(MOVE_WARPS * 32) k_move(const MoveArgs A) {
                 Ni += __popc(vm & 0x55555555u);   Npi += __popc(vm & 0xAAAAAAAAu);
                 Npins += __popc(fm & 0x55555555u); Nins += __popc(fm & 0xAAAAAAAAu);
               }
-              cbre += ne;
+              cbre += rosen ? ne - 1u : ne;
               if (Npins == 0) { zero = true; needed = kk + 1u; break; }
-              const float wk = __fdiv_rn((float)(Npins * (Npi + 1u)), (float)((Nins + 1u) * Ni));
+              const float wk = rosen ? __fdiv_rn((float)Npins, (float)(Nins + 1u))
+                                     : __fdiv_rn((float)(Npins * (Npi + 1u)), (float)((Nins + 1u) * Ni));
               P = P * wk;
             }
           }

@@ -179,6 +179,8 @@ struct QTables {
   uint32_t* knext; uint32_t* rejmin; const int* head; uint32_t* todo; const uint16_t* alive;
   // configurational bias: job list of the current window
   uint32_t* jk; uint32_t* jm; uint2* jc; int* jhead; uint32_t* njobs; int jcap;
+  // OPT_SHELL (R-N1): depletants in the shell R_in < |d| <= R instead of the whole ball
+  float sh_Rin3, sh_dR3;
 };
 
 #ifndef HPMC_LANES_PER_OPEN_MOVE
@@ -188,7 +190,7 @@ struct QTables {
 // Phase 2 (a8): the depletant item queue over the `nalive` surviving moves described by `tb`; returns when no move
 // of the tile has unclaimed work left and this thread's last item is done.  rejmin[m] starts at N_d and only
 // decreases, so "k < rejmin[m]" is the one test for "this depletant still matters".
-template <int SHAPE, bool CB>
+template <int SHAPE, bool CB, bool SHELL>
 __device__ __forceinline__ void q_depletant_queue(const QTables& tb, int nalive, const Geo& g, const Key10& key,
                                                   uint32_t c3dep, int t, uint32_t& n_eval, uint32_t& n_blocks) {
   constexpr bool ANISO = SHAPE != SH_SPHERE;
@@ -255,10 +257,19 @@ __device__ __forceinline__ void q_depletant_queue(const QTables& tb, int nalive,
       // one Philox block = one cube-rejection attempt of depletant k (R-S3); c3 carries the attempt number
       const Block4 r = philox(key, c_pid, k, 0, c3);
       ++n_blocks;
-      V3 d = V3{g.Rins * sym_unit_bits(r.x), g.Rins * sym_unit_bits(r.y), g.Rins * sym_unit_bits(r.z)};
-      float d2 = dot3(d, d);
-      bool inside = d2 <= g.Rins2;
-      if (!inside && c3 >= c3dep + (63u << 16)) { d = V3{0.f, 0.f, 0.f}; d2 = 0.0f; inside = true; }
+      V3 d;
+      float d2;
+      bool inside;
+      if (!SHELL) {
+        d = V3{g.Rins * sym_unit_bits(r.x), g.Rins * sym_unit_bits(r.y), g.Rins * sym_unit_bits(r.z)};
+        d2 = dot3(d, d);
+        inside = d2 <= g.Rins2;
+        if (!inside && c3 >= c3dep + (63u << 16)) { d = V3{0.f, 0.f, 0.f}; d2 = 0.0f; inside = true; }
+      } else {
+        inside = shell_attempt(r, tb.sh_Rin3, tb.sh_dR3, d);
+        if (!inside && c3 >= c3dep + (63u << 16)) { d = V3{g.Rins, 0.f, 0.f}; inside = true; }
+        d2 = inside ? dot3(d, d) : 0.0f;
+      }
       if (inside) {
         ++n_eval;
         const V3 ro = V3{c_rho.x, c_rho.y, c_rho.z};
@@ -614,7 +625,9 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
       QTables tb;
       tb.r1 = s_r1; tb.rho = s_rho; tb.aold = s_aold; tb.anew = s_anew; tb.pool = s_pool;
       tb.knext = s_knext; tb.rejmin = s_rejmin; tb.head = s_head; tb.todo = s_todo; tb.alive = s_alive;
-      q_depletant_queue<SHAPE, false>(tb, nalive, g, A.key, c3dep, t, n_eval, n_blocks);
+      tb.sh_Rin3 = A.sh_Rin3; tb.sh_dR3 = A.sh_dR3;
+      if (A.options & OPT_SHELL) q_depletant_queue<SHAPE, false, true>(tb, nalive, g, A.key, c3dep, t, n_eval, n_blocks);
+      else q_depletant_queue<SHAPE, false, false>(tb, nalive, g, A.key, c3dep, t, n_eval, n_blocks);
     }
     __syncthreads();
     } else {
@@ -626,6 +639,8 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
     // (R-G3), which also fixes dep_needed and the reinsertion count exactly as the sequential definition does.
     const uint32_t ne = 2u * (uint32_t)A.n_trial;
     const uint32_t c3cb = P_CBPOS + colw;
+    // OPT_ROSENBLUTH (R-N4): weight N'_ins / (N_ins + 1), the last reverse reinsertion is not drawn
+    const bool rosen = (A.options & OPT_ROSENBLUTH) != 0u;
     uint32_t W = HPMC_CB_WINDOW;
     for (int e = t; e < nlist; e += T) { s_P[e] = 1.0f; s_cbre[e] = 0u; s_klo[e] = 0u; }
     __syncthreads();
@@ -652,7 +667,9 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
         tb.r1 = s_r1; tb.rho = s_rho; tb.aold = s_aold; tb.anew = s_anew; tb.pool = s_pool;
         tb.knext = s_knext; tb.rejmin = s_rejmin; tb.head = s_head; tb.todo = s_todo; tb.alive = s_alive;
         tb.jk = s_jk; tb.jm = s_jm; tb.jc = s_jc; tb.jhead = s_jhead; tb.njobs = &s_scal[5]; tb.jcap = S::JCAP;
-        q_depletant_queue<SHAPE, true>(tb, nalive, g, A.key, c3dep, t, n_eval, n_blocks);
+        tb.sh_Rin3 = A.sh_Rin3; tb.sh_dR3 = A.sh_dR3;
+        if (A.options & OPT_SHELL) q_depletant_queue<SHAPE, true, true>(tb, nalive, g, A.key, c3dep, t, n_eval, n_blocks);
+        else q_depletant_queue<SHAPE, true, false>(tb, nalive, g, A.key, c3dep, t, n_eval, n_blocks);
       }
       __syncthreads();
       const uint32_t njobs = s_scal[5];
@@ -668,6 +685,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
         const uint32_t jb = i / ne, e2 = i - jb * ne;
         const uint32_t m = s_jm[jb] & 0xffffu, kk = s_jk[jb];
         const uint32_t dir = e2 & 1u, tt = e2 >> 1;
+        if (rosen && e2 == ne - 1u) continue;
         const float4 r1f = s_r1[m], rof = s_rho[m];
         const V3 ro = V3{rof.x, rof.y, rof.z};
         V3 ao = V3{0.f, 0.f, 1.f}, an = V3{0.f, 0.f, 1.f};
@@ -706,7 +724,8 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
           const uint32_t Ni = c.x & 0xffffu, Npins = c.x >> 16, Npi = c.y & 0xffffu, Nins = c.y >> 16;
           ++cbre;
           if (Npins == 0u) { zero = true; s_state[e] = OUT_CB; s_rejmin[e] = bk + 1u; break; }   // R-G3; dep_needed = k + 1
-          P = P * __fdiv_rn((float)(Npins * (Npi + 1u)), (float)((Nins + 1u) * Ni));            // Eq. 16, R-G1
+          P = P * (rosen ? __fdiv_rn((float)Npins, (float)(Nins + 1u))                           // R-N4
+                         : __fdiv_rn((float)(Npins * (Npi + 1u)), (float)((Nins + 1u) * Ni)));   // Eq. 16, R-G1
         }
         s_P[e] = P; s_cbre[e] = cbre;
         if (!zero) s_klo[e] = s_rejmin[e];     // window end
@@ -733,7 +752,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
         const uint32_t Nd = s_Nd[e], cbre = s_cbre[e];
         atomicAdd(&s_cnt[C_DEP_DRAWN], Nd);
         atomicAdd(&s_cnt[C_DEP_NEEDED], out == OUT_CB ? s_rejmin[e] : Nd);
-        if (cbre) atomicAdd(&s_cnt[C_CB_REINSERTIONS], cbre * 2u * (uint32_t)A.n_trial);
+        if (cbre) atomicAdd(&s_cnt[C_CB_REINSERTIONS], cbre * (2u * (uint32_t)A.n_trial - ((A.options & OPT_ROSENBLUTH) ? 1u : 0u)));
         if (out == OUT_NONE) {
           if (cbre == 0u) out = OUT_ACCEPT;          // no rejecting depletant at all
           else {

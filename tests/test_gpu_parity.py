@@ -37,9 +37,12 @@ def _bits(a):
     return np.ascontiguousarray(a).view(np.uint32)
 
 
-def run_parity(cfg, pos, quat, sweeps, n_R, step0=0, check_cells_every=10):
+def run_parity(cfg, pos, quat, sweeps, n_R, step0=0, check_cells_every=10, options=0):
     o, h, dpos, dquat = _mk(cfg, pos, quat)
     assert (o.n_c, np.float32(o.w)) == (h.n_c, np.float32(h.w))
+    if options:
+        o.set_flags(options)          # same bit values on both sides: 1 shell (R-N1), 2 Rosenbluth weight (R-N4)
+        h.set_options(options)
     for s in range(step0, step0 + sweeps):
         o.build_cells(cfg.seed, s)
         h.build_cells(cfg.seed, s)
@@ -140,6 +143,39 @@ def test_configurational_bias_through_the_item_queue_kernel(monkeypatch, name, N
     cfg = dataclasses.replace(workloads.config(name, N), n_trial=n_trial)
     pos, quat = workloads.generate(cfg)
     c = run_parity(cfg, pos, quat, sweeps if FULL else 15, cfg.n_R())
+    assert c["cb_reinsertions"] > 0 and c["rej_cb"] > 0
+
+
+@pytest.mark.parametrize("name,N,sweeps,d_max", [("C1", None, 100, None), ("C2", 16384, 60, None), ("C3", 65536, 30, None),
+                                                 ("C3", 16384, 30, 0.0005), ("C4", 4096, 40, None)])
+def test_shell_restricted_insertion_volume(name, N, sweeps, d_max):
+    """HPMC_OPT_SHELL (reading R-N1): depletants drawn in the shell
+    R_in < |d| <= R, N_d ~ Poisson(n_R V_shell).  Bit parity of outcomes, poses and counters as for the default path;
+    the small-step case has a thin shell (R_in / R = 0.998), the half-balls R_in = 0 (the whole ball through the shell
+    sampler)."""
+    import dataclasses
+    cfg = workloads.config(name, N)
+    if d_max is not None:
+        cfg = dataclasses.replace(cfg, d_max=d_max)
+    pos, quat = workloads.generate(cfg)
+    c = run_parity(cfg, pos, quat, sweeps if FULL else 10, cfg.n_R(), options=1)
+    assert c["dep_drawn"] > 0 and c["rej_depletant"] > 0
+    if d_max is not None:
+        assert c["accept_trans"] > 0.1 * c["trials_trans"]
+
+
+@pytest.mark.parametrize("kernel", ["warp", "queue"])
+@pytest.mark.parametrize("name,N,n_trial,options,sweeps", [("C5", None, 4, 2, 100), ("C5", 4096, 10, 2, 40),
+                                                           ("C1", None, 4, 3, 100), ("C4", 4096, 1, 2, 40)])
+def test_rosenbluth_weight_option(monkeypatch, kernel, name, N, n_trial, options, sweeps):
+    """HPMC_OPT_ROSENBLUTH (NEXT-4, reading R-N4): weight N'_ins / (N_ins + 1), n_trial forward and n_trial - 1 reverse
+    reinsertions; through both CB kernels, alone and together with the shell option, down to n_trial = 1 (no reverse
+    reinsertion at all)."""
+    import dataclasses
+    monkeypatch.setenv("HPMC_CB_KERNEL", kernel)
+    cfg = dataclasses.replace(workloads.config(name, N), n_trial=n_trial)
+    pos, quat = workloads.generate(cfg)
+    c = run_parity(cfg, pos, quat, sweeps if FULL else 10, cfg.n_R(), options=options)
     assert c["cb_reinsertions"] > 0 and c["rej_cb"] > 0
 
 
