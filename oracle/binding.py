@@ -91,6 +91,7 @@ def lib() -> C.CDLL:
                 "oracle_eval_move": (i32, [vp, u32, u32, i64, vp, vp, f64, i32]),
                 "oracle_eval_moves": (i32, [vp, u32, u32, i64, i64, vp, vp, f64, i32, vp]),
                 "oracle_count_overlaps": (i64, [vp, i32]),
+                "oracle_free_volume": (i32, [vp, u32, u32, i64, vp]),
                 "oracle_philox4x32_10": (None, [vp, vp, vp]),
                 "oracle_unit01": (f32, [u32]),
                 "oracle_sym_unit": (f32, [u32]),
@@ -208,6 +209,14 @@ class Oracle:
         if rc:
             raise RuntimeError("oracle_eval_moves rc=%d" % rc)
         return out
+
+    def free_volume(self, seed, step, n):
+        """Number of n uniform test depletants that overlap no colloid (needs build_cells(seed, step))."""
+        out = np.zeros(1, np.uint64)
+        rc = self.L.oracle_free_volume(self.h, seed, step, int(n), _ptr(out))
+        if rc:
+            raise RuntimeError("oracle_free_volume rc=%d" % rc)
+        return int(out[0])
 
     def count_overlaps(self, both_ways=True):
         return int(self.L.oracle_count_overlaps(self.h, 1 if both_ways else 0))

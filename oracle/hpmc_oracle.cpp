@@ -71,7 +71,7 @@ static inline U4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c
 }
 
 // stream purposes, R-S20
-enum { P_SWEEP = 0, P_SELECT = 1, P_MOVE = 2, P_NDEP = 3, P_DEPPOS = 4, P_CBPOS = 5, P_ACCEPT = 6 };
+enum { P_SWEEP = 0, P_SELECT = 1, P_MOVE = 2, P_NDEP = 3, P_DEPPOS = 4, P_CBPOS = 5, P_ACCEPT = 6, P_FREEVOL = 7 };
 
 static inline uint32_t word3(uint32_t purpose, uint32_t colour, uint32_t attempt) {
   return purpose + (colour << 8) + (attempt << 16);
@@ -772,6 +772,40 @@ int oracle_eval_moves(void* h, uint32_t seed, uint32_t draw0, int64_t n, int64_t
     out[j] = outside ? (uint8_t)OUT_BOUNDARY
                      : (uint8_t)evaluate_move(*c, seed, draw0 + (uint32_t)j, 0, i, own, r0, q0, r1, q1, n_trial, dm, cn);
   }
+  return 0;
+}
+
+// Free-volume measurement (Sec. IV.A, Fig. 4: the depletant density in the
+// system is n_R times the free-volume fraction): n test depletants at points uniform in the box, sample s from Philox
+// block (s mod 2^32, s / 2^32, 0, FREEVOL) of key (seed, step), x_a = unit01(word a) L; counted if it overlaps no
+// colloid (the insertion kernel's own predicate against the 27 cells around the point; cell width >= 2 R covers the
+// range).  Needs the cell list of oracle_build_cells(seed, step).
+int oracle_free_volume(void* h, uint32_t seed, uint32_t step, int64_t n, uint64_t* free_count) {
+  Ctx* c = (Ctx*)h;
+  if (!c->built || c->b_seed != seed || c->b_step != step) return -3;
+  const Geo& g = c->g;
+  const int nc = c->nc;
+  uint64_t cnt = 0;
+#pragma omp parallel for schedule(static) reduction(+ : cnt)
+  for (int64_t s = 0; s < n; ++s) {
+    const U4 r = philox4x32_10((uint32_t)((uint64_t)s & 0xffffffffu), (uint32_t)((uint64_t)s >> 32), 0,
+                               word3(P_FREEVOL, 0, 0), seed, step);
+    const V3 p = V3{unit01(r.v[0]) * g.L, unit01(r.v[1]) * g.L, unit01(r.v[2]) * g.L};
+    const int ix = cell_axis(*c, p.x, c->shift[0]), iy = cell_axis(*c, p.y, c->shift[1]), iz = cell_axis(*c, p.z, c->shift[2]);
+    bool is_free = true;
+    for (int dz = -1; dz <= 1 && is_free; ++dz)
+      for (int dy = -1; dy <= 1 && is_free; ++dy)
+        for (int dx = -1; dx <= 1 && is_free; ++dx) {
+          const int jx = (ix + dx + nc) % nc, jy = (iy + dy + nc) % nc, jz = (iz + dz + nc) % nc;
+          const int64_t cj = ((int64_t)jz * nc + jy) * nc + jx;
+          for (uint32_t t = c->cell_start[(size_t)cj]; t < c->cell_start[(size_t)cj + 1]; ++t) {
+            const int64_t j = c->cell_pid[t];
+            if (dep_overlap(g, minimg(g, p, load_r(*c, j)), quat_axis(load_q(*c, j)))) { is_free = false; break; }
+          }
+        }
+    cnt += is_free ? 1u : 0u;
+  }
+  *free_count = cnt;
   return 0;
 }
 

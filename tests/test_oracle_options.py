@@ -175,3 +175,58 @@ def test_flags_zero_is_the_default_path_and_options_keep_the_invariants():
     per_move_s = cs["dep_drawn"] / (cs["trials_trans"] - cs["rej_boundary"] - cs["rej_hard"])
     per_move_a = ca["dep_drawn"] / (ca["trials_trans"] - ca["rej_boundary"] - ca["rej_hard"])
     assert abs(per_move_s / per_move_a / frac - 1.0) < 0.02
+
+
+# ------------------------------------------------------------------ free-volume measurement (Fig. 4)
+def _free_fraction(shape, pos, quat, L, sigma_d, n, disk=(0.0, 0.0)):
+    p4 = np.zeros((len(pos), 4), np.float32)
+    p4[:, :3] = pos
+    o = oracle.Oracle(shape, 1.0, sigma_d, L, 0.1, p4, quat, *disk, threads=os.cpu_count() or 1)
+    o.build_cells(3, 9)
+    return o.free_volume(3, 9, n) / n
+
+
+def test_free_volume_closed_forms():
+    """Fraction of uniform test depletants that overlap no colloid = 1 - (excluded volume) / V: one sphere (4 pi R^3/3),
+    two spheres with overlapping exclusion spheres (minus the lens, ref. 17), one half-ball and one spherodisk
+    (Steiner volumes 0.557698 and 0.319281), 3 sigma at 2e6 points."""
+    n, L = 2000000, 6.0
+    V = L ** 3
+    Vs = 4.0 * math.pi * 0.6 ** 3 / 3.0
+    q = np.array([[0.3, -0.5, 0.2, 0.78]], np.float32)
+    q /= np.linalg.norm(q)
+    cases = [("sphere", [[1.0, 2.0, 3.0]], None, 0.2, (0.0, 0.0), Vs),
+             ("sphere", [[1.0, 2.0, 3.0], [2.05, 2.0, 3.0]], None, 0.2, (0.0, 0.0), 2.0 * Vs - lens(0.6, 1.05)),
+             ("sphere", [[5.9, 0.1, 3.0]], None, 0.2, (0.0, 0.0), Vs),                      # across the periodic boundary
+             ("halfball", [[1.0, 2.0, 3.0]], q, 0.2, (0.0, 0.0), 0.557698),
+             ("spherodisk", [[1.0, 2.0, 3.0]], q, 0.15, (0.4, 0.1), 0.319281)]
+    for shape, pos, quat, sd, disk, vexcl in cases:
+        got = _free_fraction(shape, pos, quat, L, sd, n, disk)
+        want = 1.0 - vexcl / V
+        assert abs(got - want) < 3.0 * math.sqrt(want * (1 - want) / n) + 1e-6, (shape, got, want)
+
+
+def test_free_volume_equals_brute_force_on_the_same_points():
+    """C1 (256 spheres): the same Philox points (rebuilt here from the separately pinned block function and u32->float map)
+    against all 256 centres in numpy fp64 with the minimum image; equal counts up to points within 1e-6 of a surface."""
+    cfg = workloads.config("C1")
+    pos, _ = workloads.generate(cfg)
+    o = oracle.Oracle("sphere", 1.0, cfg.sigma_d, cfg.box_L, cfg.d_max, pos, threads=os.cpu_count() or 1)
+    o.build_cells(7, 2)
+    n = 40000
+    got = o.free_volume(7, 2, n)
+    L_ = oracle.lib()
+    pts = np.zeros((n, 3))
+    ctr, key, out = np.zeros(4, np.uint32), np.array([7, 2], np.uint32), np.zeros(4, np.uint32)
+    for s in range(n):
+        ctr[:] = (s, 0, 0, 7)                    # purpose FREEVOL = 7, colour 0, attempt 0
+        L_.oracle_philox4x32_10(_vp(ctr), _vp(key), _vp(out))
+        pts[s] = [np.float32(L_.oracle_unit01(int(out[a]))) * np.float32(cfg.box_L) for a in range(3)]
+    Lb = float(np.float32(cfg.box_L))
+    d = pts[:, None, :] - pos[None, :, :3].astype(np.float64)
+    d -= Lb * np.round(d / Lb)
+    r = np.sqrt((d ** 2).sum(axis=2)).min(axis=1)
+    R = 0.5 * (1.0 + cfg.sigma_d)
+    free, border = int((r >= R).sum()), int((np.abs(r - R) < 1e-6).sum())
+    assert abs(got - free) <= border, (got, free, border)
+    assert 0.6 * n < got < 0.95 * n
