@@ -132,6 +132,14 @@ int hpmc_run(hpmc_ctx* ctx, uint32_t seed, uint32_t step0, int64_t n_sweeps, dou
 int hpmc_counters(hpmc_ctx* ctx, hpmc_counters_t* host_out);
 int hpmc_reset_counters(hpmc_ctx* ctx);
 
+/* Free-volume measurement (Sec. IV.A, Fig. 4: the depletant density in the system
+ * is n_R times the free-volume fraction).  n_samples test depletants at points uniform in the box -- sample s from the
+ * Philox block (s mod 2^32, s / 2^32, 0, FREEVOL = 7) of key (seed, step), x_a = unit01(word a) box_L -- are tested with
+ * the insertion kernel's own predicate against the 27 cells around the point; *host_free_count = how many overlap no
+ * colloid, so free-volume fraction = count / n_samples.  Needs hpmc_build_cells(seed, step) (else HPMC_E_STATE) and may
+ * be called before or instead of hpmc_sweep.  Synchronises the stream. */
+int hpmc_free_volume(hpmc_ctx* ctx, uint32_t seed, uint32_t step, int64_t n_samples, uint64_t* host_free_count);
+
 /* Copy the outcome codes of the last sweep into d_outcome (device, N bytes, caller-owned).  Asynchronous.
  * hpmc_build_cells resets the codes to HPMC_OUT_NONE for the sweep it prepares. */
 int hpmc_outcomes(hpmc_ctx* ctx, uint8_t* d_outcome);

@@ -22,7 +22,7 @@ EXPORTS = (
     "hpmc_init", "hpmc_destroy", "hpmc_build_cells", "hpmc_sweep", "hpmc_run", "hpmc_counters",
     "hpmc_reset_counters", "hpmc_outcomes", "hpmc_grid", "hpmc_cells", "hpmc_upload", "hpmc_download",
     "hpmc_step_host", "hpmc_launch_count", "hpmc_time_move_kernel", "hpmc_move_kernel_ms", "hpmc_last_error",
-    "hpmc_alu_peaks", "hpmc_set_options",
+    "hpmc_alu_peaks", "hpmc_set_options", "hpmc_free_volume",
 )
 
 
@@ -77,6 +77,7 @@ def load_library() -> C.CDLL:
         "hpmc_sweep": (i32, [vp, u32, u32, f64, f32, f32, i32]),
         "hpmc_run": (i32, [vp, u32, u32, i64, f64, f32, f32, i32]),
         "hpmc_set_options": (i32, [vp, u32]),
+        "hpmc_free_volume": (i32, [vp, u32, u32, i64, P(C.c_uint64)]),
         "hpmc_counters": (i32, [vp, P(Counters)]),
         "hpmc_reset_counters": (i32, [vp]),
         "hpmc_outcomes": (i32, [vp, vp]),
@@ -170,6 +171,11 @@ class HPMC:
 
     def sweep(self, seed, step, n_R, d_max, a_max=0.0, n_trial=0):
         self._ck(self.L.hpmc_sweep(self.h, seed, step, float(n_R), d_max, a_max, n_trial))
+
+    def free_volume(self, seed, step, n_samples):
+        out = C.c_uint64(0)
+        self._ck(self.L.hpmc_free_volume(self.h, seed, step, int(n_samples), C.byref(out)))
+        return int(out.value)
 
     def set_options(self, options):
         self._ck(self.L.hpmc_set_options(self.h, int(options)))

@@ -589,6 +589,35 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
   return HPMC_OK;
 }
 
+int hpmc_free_volume(hpmc_ctx* ctx, uint32_t seed, uint32_t step, int64_t n_samples, uint64_t* host_free_count) {
+  if (!ctx || !host_free_count || n_samples < 0) return HPMC_E_BADARG;
+  if (!ctx->built || ctx->b_seed != seed || ctx->b_step != step)
+    return fail(ctx, HPMC_E_STATE, "hpmc_free_volume: call hpmc_build_cells(seed, step) first");
+  unsigned long long* d_cnt = nullptr;
+  CU(cudaMalloc(&d_cnt, sizeof(unsigned long long)));
+  CU(cudaMemsetAsync(d_cnt, 0, sizeof(unsigned long long), ctx->stream));
+  if (n_samples > 0) {
+    const Key10 key = make_key(seed, step);
+    long long blocks = (n_samples + 255) / 256;
+    const long long cap = (long long)ctx->num_sms * 16;
+    if (blocks > cap) blocks = cap;
+    const dim3 grid((unsigned)blocks);
+    switch (ctx->p.shape) {
+      case HPMC_SPHERE: k_free_volume<SH_SPHERE><<<grid, 256, 0, ctx->stream>>>(ctx->g, key, ctx->shift[0], ctx->shift[1], ctx->shift[2], n_samples, ctx->d_cpos, ctx->d_caxis, ctx->d_cell_start, d_cnt); break;
+      case HPMC_HALFBALL: k_free_volume<SH_HALFBALL><<<grid, 256, 0, ctx->stream>>>(ctx->g, key, ctx->shift[0], ctx->shift[1], ctx->shift[2], n_samples, ctx->d_cpos, ctx->d_caxis, ctx->d_cell_start, d_cnt); break;
+      default: k_free_volume<SH_SPHERODISK><<<grid, 256, 0, ctx->stream>>>(ctx->g, key, ctx->shift[0], ctx->shift[1], ctx->shift[2], n_samples, ctx->d_cpos, ctx->d_caxis, ctx->d_cell_start, d_cnt); break;
+    }
+    ctx->launches += 1;
+  }
+  unsigned long long h = 0;
+  CU(cudaMemcpyAsync(&h, d_cnt, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  CU(cudaGetLastError());
+  CU(cudaFree(d_cnt));
+  *host_free_count = (uint64_t)h;
+  return HPMC_OK;
+}
+
 int hpmc_set_options(hpmc_ctx* ctx, uint32_t options) {
   if (!ctx) return HPMC_E_BADARG;
   if (options & ~(uint32_t)(HPMC_OPT_SHELL | HPMC_OPT_ROSENBLUTH)) return fail(ctx, HPMC_E_BADARG, "hpmc_set_options: unknown option bit");

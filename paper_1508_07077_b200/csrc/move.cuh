@@ -123,6 +123,48 @@ __device__ __forceinline__ bool old_only(const Geo& g, const MoveCtx<SHAPE>& m, 
   return dep_overlap<SHAPE>(g, d - m.rho_old, m.a_old) && !dep_overlap<SHAPE>(g, d, m.a_new);
 }
 
+// Free-volume measurement (hpmc_free_volume; Sec. IV.A): one test depletant per thread at a uniform point of
+// the box; free iff it overlaps no colloid of the 27 cells around it (9 x-rows, each one or two spans of the
+// cell-ordered arrays).  Integer result: a count, accumulated per warp.
+template <int SHAPE>
+__global__ void __launch_bounds__(256) k_free_volume(Geo g, Key10 key, float sx, float sy, float sz, long long n,
+                                                     const float4* __restrict__ cpos, const float4* __restrict__ caxis,
+                                                     const uint32_t* __restrict__ cell_start,
+                                                     unsigned long long* __restrict__ count) {
+  const int nc = g.nc;
+  unsigned long long mine = 0;
+  for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += (long long)gridDim.x * blockDim.x) {
+    const Block4 r = philox(key, (uint32_t)((unsigned long long)s & 0xffffffffull), (uint32_t)((unsigned long long)s >> 32), 0,
+                            ctr_word3(P_FREEVOL, 0, 0));
+    const V3 p = V3{unit01(r.x) * g.L, unit01(r.y) * g.L, unit01(r.z) * g.L};
+    const int ix = cell_axis(g, p.x, sx), iy = cell_axis(g, p.y, sy), iz = cell_axis(g, p.z, sz);
+    bool is_free = true;
+    for (int row = 0; row < 9 && is_free; ++row) {
+      int jy = iy + row % 3 - 1, jz = iz + row / 3 - 1;
+      jy += (jy < 0) ? nc : 0; jy -= (jy >= nc) ? nc : 0;
+      jz += (jz < 0) ? nc : 0; jz -= (jz >= nc) ? nc : 0;
+      const uint32_t rb = ((uint32_t)jz * nc + jy) * nc;
+      int x0 = ix - 1, n0 = 3, n1 = 0;
+      if (ix == 0) { x0 = nc - 1; n0 = 1; n1 = 2; }
+      else if (ix == nc - 1) { x0 = nc - 2; n0 = 2; n1 = 1; }
+      for (int part = 0; part < (n1 != 0 ? 2 : 1) && is_free; ++part) {
+        const uint32_t b = part == 0 ? cell_start[rb + x0] : cell_start[rb];
+        const uint32_t e = part == 0 ? cell_start[rb + x0 + n0] : cell_start[rb + n1];
+        for (uint32_t t = b; t < e; ++t) {
+          const float4 c = cpos[t];
+          V3 a = V3{0.0f, 0.0f, 1.0f};
+          if (SHAPE != SH_SPHERE) { const float4 ax = caxis[t]; a = V3{ax.x, ax.y, ax.z}; }
+          const V3 d = V3{minimg1(g, p.x - c.x), minimg1(g, p.y - c.y), minimg1(g, p.z - c.z)};
+          if (dep_overlap<SHAPE>(g, d, a)) { is_free = false; break; }
+        }
+      }
+    }
+    mine += is_free ? 1ull : 0ull;
+  }
+  for (int o = 16; o >= 1; o >>= 1) mine += __shfl_xor_sync(0xffffffffu, mine, o);
+  if ((threadIdx.x & 31) == 0 && mine) atomicAdd(count, mine);
+}
+
 template <int SHAPE, bool CB>
 __global__ void __launch_bounds__(MOVE_WARPS * 32) k_move(const MoveArgs A) {
   __shared__ int s_excl[MOVE_WARPS][32];

@@ -7,7 +7,7 @@
 
 namespace hpmc {
 
-enum : uint32_t { P_SWEEP = 0, P_SELECT = 1, P_MOVE = 2, P_NDEP = 3, P_DEPPOS = 4, P_CBPOS = 5, P_ACCEPT = 6 };
+enum : uint32_t { P_SWEEP = 0, P_SELECT = 1, P_MOVE = 2, P_NDEP = 3, P_DEPPOS = 4, P_CBPOS = 5, P_ACCEPT = 6, P_FREEVOL = 7 };
 
 struct Key10 {  // the ten round keys of one (seed, step): hoisted out of every block computation
   uint32_t k0[10], k1[10];

@@ -179,6 +179,30 @@ def test_rosenbluth_weight_option(monkeypatch, kernel, name, N, n_trial, options
     assert c["cb_reinsertions"] > 0 and c["rej_cb"] > 0
 
 
+@pytest.mark.parametrize("name,N", [("C1", None), ("C3", 65536), ("C4", None), ("C5", None)])
+def test_free_volume_measurement(name, N):
+    """hpmc_free_volume: the number of free test depletants is an integer and
+    must EQUAL the oracle's on the same Philox points, before and after a few sweeps; also the empty sample."""
+    cfg = workloads.config(name, N)
+    pos, quat = workloads.generate(cfg)
+    o, h, dpos, dquat = _mk(cfg, pos, quat)
+    n = 1000000 if FULL else 100000
+    for s in range(3):
+        o.build_cells(cfg.seed, s); h.build_cells(cfg.seed, s)
+        fo, fg = o.free_volume(cfg.seed, s, n), h.free_volume(cfg.seed, s, n)
+        assert fg == fo, (s, fg, fo)
+        assert 0.05 * n < fg < 0.95 * n
+        o.sweep(cfg.seed, s, cfg.n_R(), cfg.d_max, cfg.a_max, cfg.n_trial)
+        h.sweep(cfg.seed, s, cfg.n_R(), cfg.d_max, cfg.a_max, cfg.n_trial)
+    h.build_cells(cfg.seed, 9)
+    assert h.free_volume(cfg.seed, 9, 0) == 0
+    import paper_1508_07077_b200 as hp
+    with pytest.raises(hp.HPMCError) as e:
+        h.free_volume(cfg.seed, 8, 10)                   # no cell list for (seed, 8)
+    assert e.value.code == -3
+    h.close()
+
+
 def test_one_launch_per_pass_mode(monkeypatch):
     """HPMC_SWEEP_LAUNCHES=8: the item-queue kernel launched once per checkerboard pass (no neighbour waits) instead of
     once per sweep; same bits."""
