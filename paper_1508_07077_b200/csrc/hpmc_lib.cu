@@ -79,7 +79,7 @@ struct hpmc_ctx {
   QPlan plan[2];                       // launch plans of the item-queue move kernel: [0] plain rule, [1] configurational bias
   uint32_t options = 0;                // hpmc_set_options
   bool use_queue = true;               // HPMC_MOVE_KERNEL=warp selects the first (warp-per-cell) design
-  bool cb_queue = false;               // HPMC_CB_KERNEL=queue: configurational bias through the item-queue kernel too
+  int cb_kernel = 0;                   // configurational bias: 0 = choose per sweep (n_trial, N), 1 = warp-per-cell kernel, 2 = item-queue kernel (HPMC_CB_KERNEL=warp|queue)
   int64_t launches = 0;
 #ifdef HPMC_PHASE_CLOCKS
   unsigned long long* d_phase_clk = nullptr;   // tuning build: per-phase clock sums of the move kernel (printed by hpmc_destroy)
@@ -418,11 +418,13 @@ int hpmc_init(hpmc_ctx** out, const hpmc_params* p, int64_t N, float* d_pos4, fl
   {
     const char* sel = getenv("HPMC_MOVE_KERNEL");
     ctx->use_queue = !(sel && std::string(sel) == "warp");
-    // Configurational bias runs on the warp-per-cell kernel by default: measured on spherodisks with n_trial = 4 it is
-    // 1.2-1.75x faster than the round-based CB stage of the item-queue kernel at every size tried (32,768 ... 884,736
-    // particles; profiles/r2_cb_kernels.md).  Both give the same bits and both are covered by the parity tests.
+    // Configurational bias: two kernels, same bits, both covered by the parity tests.  Measured on spherodisks
+    // (profiles/r2_cb_kernels.md): the warp-per-cell kernel wins for few reinsertions on small systems (n_trial = 4,
+    // 32,768 particles: 252 against 480 us per sweep), the item-queue kernel, which spreads the 2 n_trial reinsertions of
+    // every rejecting depletant over the whole CTA, from n_trial ~ 16 on (n_trial = 40: 1.6 against 2.2 ms; 100: 3.3
+    // against 4.8 ms) and on large systems (262,144 particles: 813 against 830 us at n_trial = 4).
     const char* cbk = getenv("HPMC_CB_KERNEL");
-    ctx->cb_queue = cbk && std::string(cbk) == "queue";
+    ctx->cb_kernel = (cbk && std::string(cbk) == "queue") ? 2 : ((cbk && std::string(cbk) == "warp") ? 1 : 0);
     int rc = 0;
     switch (p->shape) {
       case HPMC_SPHERE: rc = setup_moveq<SH_SPHERE, false>(ctx); if (!rc) rc = setup_moveq<SH_SPHERE, true>(ctx); break;
@@ -555,7 +557,8 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
     CU(cudaEventRecord(ep->a, ctx->stream));
   }
   int nlaunch = 8;
-  if (ctx->use_queue && (!cb || ctx->cb_queue)) {
+  const bool cb_queue = ctx->cb_kernel == 2 || (ctx->cb_kernel == 0 && (n_trial >= 16 || ctx->N >= 200000));
+  if (ctx->use_queue && (!cb || cb_queue)) {
     // item-queue kernel (moveq.cuh): one cooperative launch for the 8 passes (CTAs synchronise with their spatial
     // neighbours only), or one launch per pass
     const bool one = ctx->plan[cb ? 1 : 0].one_launch;
