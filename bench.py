@@ -174,10 +174,11 @@ def oracle_sample(cfg, pos, quat, sweeps, step0, min_seconds=0.0, max_sweeps=Non
     return o, c, times, oracle.lib().oracle_get_threads()
 
 
-def workload_desc(cfg):
+def workload_desc(cfg, phi=None):
+    phi = cfg.phi_d_r[0] if phi is None else phi
     return ("%s: %d hard %ss, phi_c=%.2f, q=%.2f, phi_d^r=%.2f (lambda=%.0f depletants drawn/move), d_max=%.3g, "
-            "a_max=%.3g, n_trial=%d" % (cfg.name, cfg.N, cfg.shape, cfg.phi_c, cfg.q, cfg.phi_d_r[0], cfg.lam, cfg.d_max,
-                                        cfg.a_max, cfg.n_trial))
+            "a_max=%.3g, n_trial=%d" % (cfg.name, cfg.N, cfg.shape, cfg.phi_c, cfg.q, phi, cfg.lam * phi / cfg.phi_d_r[0],
+                                        cfg.d_max, cfg.a_max, cfg.n_trial))
 
 
 def run_reference(args, cfg):
@@ -237,7 +238,8 @@ def roofline_block(cfg, c, n_c, passes, launches, kernel_ms, step_ms_total, alu,
     issue_peak = sms * LANES_PER_SM_PER_CLK * hz
     seen_mhz = clocks.get("sm_mhz") or pk["sm_max_mhz"]
     traffic, traffic_src = ncu_traffic(workload_key)
-    cb_warp = cfg.n_trial > 0 and os.environ.get("HPMC_CB_KERNEL") != "queue"
+    cbk = os.environ.get("HPMC_CB_KERNEL")        # the library's rule (hpmc_lib.cu): item queue iff n_trial >= 16 or N >= 200000
+    cb_warp = cfg.n_trial > 0 and (cbk == "warp" or (cbk != "queue" and cfg.n_trial < 16 and cfg.N < 200000))
     kern = ("k_move<%s,cb> (warp per cell, 8 launches per sweep)" % cfg.shape if cb_warp else
             "k_moveq<%s,%s> (item queue, %d launch%s per sweep)" % (cfg.shape, "cb" if cfg.n_trial > 0 else "plain",
                                                                      round(launches / max(1, passes / 8)),
@@ -263,12 +265,15 @@ def roofline_block(cfg, c, n_c, passes, launches, kernel_ms, step_ms_total, alu,
     }
 
 
-def timed_run(hp, torch, cfg, seed, pos, quat, n_R, steps, warmup, flush, step0=0):
+def timed_run(hp, torch, cfg, seed, pos, quat, n_R, steps, warmup, flush, step0=0, options=0, free_volume_samples=0):
     """`warmup` untimed + `steps` timed sweeps of one configuration from the given poses; returns the counters of the
-    timed sweeps, per-step event times, the move kernel's event time and launch count, the grid size."""
+    timed sweeps, per-step event times, the move kernel's event time and launch count, the grid size, the poses before
+    and after the timed sweeps and (free_volume_samples > 0) the free-volume fraction of the final configuration."""
     dpos = torch.from_numpy(pos.copy()).cuda()
     dquat = None if quat is None else torch.from_numpy(quat.copy()).cuda()
     h = hp.HPMC(cfg.shape, cfg.sigma_c, cfg.sigma_d, cfg.box_L, cfg.d_max, dpos, dquat, cfg.disk_a, cfg.disk_s)
+    if options:
+        h.set_options(options)
 
     def step(s):
         h.build_cells(seed, s)
@@ -277,6 +282,7 @@ def timed_run(hp, torch, cfg, seed, pos, quat, n_R, steps, warmup, flush, step0=
     for s in range(warmup):
         step(step0 + s)
     torch.cuda.synchronize()
+    start_pos = dpos.cpu().numpy()
     h.reset_counters()
     l0 = h.launch_count()
     h.time_move_kernel(True)
@@ -295,7 +301,11 @@ def timed_run(hp, torch, cfg, seed, pos, quat, n_R, steps, warmup, flush, step0=
     h.time_move_kernel(False)
     c = h.counters()
     out = dict(c=c, step_ms=step_ms, kernel_ms=kms, kernel_launches=kl, launches=h.launch_count() - l0, n_c=h.n_c,
-               final_pos=dpos.cpu().numpy(), final_quat=None if dquat is None else dquat.cpu().numpy())
+               start_pos=start_pos, final_pos=dpos.cpu().numpy(), final_quat=None if dquat is None else dquat.cpu().numpy())
+    if free_volume_samples:
+        s_fv = step0 + warmup + steps
+        h.build_cells(seed, s_fv)
+        out["free_volume_fraction"] = h.free_volume(seed, s_fv, free_volume_samples) / free_volume_samples
     h.close()
     return out
 
@@ -304,9 +314,10 @@ def per_config_lines(hp, torch, alu, pk, flush, clocks):
     """moves/s, depletant insertions/s, us per pass and roofline fraction of the other BASELINE.json configurations
     (C1, C2 at its four reservoir densities after melting 1000 sweeps at n_R = 0 through the library, C4, C5), each a
     short device-timed run from its seeded initial state.  Context for the C3 headline, same kernels, same clocks."""
+    import numpy as np
     out = {}
-    plan = [("C1", None, 200), ("C2", None, 50), ("C4", None, 50), ("C5", None, 50)]
-    for name, _, steps in plan:
+    plan = [("C1", 200, 0), ("C2", 50, 0), ("C4", 50, 0), ("C5", 50, 0), ("C3", 10, hp.OPT_SHELL)]
+    for name, steps, options in plan:
         cfg = workloads.config(name)
         pos, quat = workloads.generate(cfg)
         dens = [(None, cfg.n_R())]
@@ -315,21 +326,29 @@ def per_config_lines(hp, torch, alu, pk, flush, clocks):
             pos = m["final_pos"]
             dens = [(phi, cfg.n_R(phi)) for phi in cfg.phi_d_r]
         for phi, n_R in dens:
-            r = timed_run(hp, torch, cfg, cfg.seed, pos, quat, n_R, steps, 5, flush)
+            r = timed_run(hp, torch, cfg, cfg.seed, pos, quat, n_R, steps, 5, flush, options=options,
+                          free_volume_samples=1000000)
             c = r["c"]
             tot_s = sum(r["step_ms"]) * 1e-3
             moves = c["trials_trans"] + c["trials_rot"]
             rf = roofline_block(cfg, c, r["n_c"], 8 * steps, r["kernel_launches"], r["kernel_ms"], sum(r["step_ms"]), alu, pk,
-                                clocks, name)
+                                clocks, name if not options else None)
+            # mean-square displacement over the timed sweeps per wall-clock second (Fig. 8's figure of merit, L240)
+            dr = (r["final_pos"][:, :3].astype(np.float64) - r["start_pos"][:, :3].astype(np.float64))
+            dr -= cfg.box_L * np.round(dr / cfg.box_L)
+            msd = float((dr ** 2).sum(axis=1).mean())
             key = name if phi is None else "%s phi_d^r=%.1f" % (name, phi)
+            if options:
+                key += " HPMC_OPT_SHELL"
             out[key] = {
-                "workload": workload_desc(cfg) if phi is None else workload_desc(cfg).replace(
-                    "phi_d^r=%.2f" % cfg.phi_d_r[0], "phi_d^r=%.2f" % phi),
+                "workload": workload_desc(cfg, phi) + (" + HPMC_OPT_SHELL (R-N1)" if options else ""),
                 "moves_per_s": moves / tot_s, "dep_needed_per_s": c["dep_needed"] / tot_s,
                 "dep_evaluated_per_s": c["dep_evaluated"] / tot_s, "dep_drawn_per_s": c["dep_drawn"] / tot_s,
                 "ms_per_step": 1e3 * tot_s / steps, "us_per_pass": rf["us_per_pass"], "acceptance":
                 (c["accept_trans"] + c["accept_rot"]) / max(1, moves), "roofline_frac": rf["frac"],
                 "frac_of_issue_bound": rf["frac_of_issue_bound"], "kernel": rf["kernel"], "steps": steps,
+                "dep_needed_per_move": c["dep_needed"] / max(1, moves), "dep_drawn_per_move": c["dep_drawn"] / max(1, moves),
+                "free_volume_fraction": r.get("free_volume_fraction"), "msd_per_s": msd / tot_s, "msd_per_sweep": msd / steps,
             }
     return out
 

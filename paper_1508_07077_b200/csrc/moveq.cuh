@@ -487,7 +487,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
           asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(Q.done + b) : "memory");
           if ((int32_t)(v - target) >= 0) break;
           if (++spins > (1u << 20)) { atomicExch(A.err_flag, 2); break; }
-          __nanosleep(spins < 4u ? 100u : 400u);      // polls cost issue slots of the SM's other CTAs: back off
+          __nanosleep(spins < 64u ? 40u : 200u);      // short waits are the rule (small systems are latency-bound); back off on long ones
         }
         polled = true;
       }
