@@ -118,7 +118,7 @@ static inline Q4 rotate_cayley(Q4 q, V3 v) {
 }
 
 // ----------------------------------------------------------------------------- shapes
-enum { SH_SPHERE = 0, SH_HALFBALL = 1, SH_SPHERODISK = 2 };
+enum { SH_SPHERE = 0, SH_HALFBALL = 1, SH_SPHERODISK = 2, SH_ELLIPSOID = 3 };
 
 struct Geo {                 // derived fp32 constants, R-0
   int shape;
@@ -129,7 +129,7 @@ struct Geo {                 // derived fp32 constants, R-0
   float rcut2;               // neighbour pre-filter
   float Rh;                  // half-ball radius
   float cen;                 // half-ball interior-point offset 3Rh/8
-  float adisk, sdisk;        // spherodisk: disk radius, rounding radius
+  float adisk, sdisk;        // spherodisk: disk radius, rounding radius; ellipsoid: equatorial and polar semi-axes A >= C
   float rs2;                 // (sdisk+rd)^2
   float rd2;                 // rd^2
 };
@@ -154,13 +154,41 @@ static Geo make_geo(int shape, float sigma_c, float disk_a, float disk_s, float 
   return g;
 }
 
+// R-N2 (the paper's discoids are oblate ellipsoids a = b = 0.5, c = 0.25, L228): is the point at
+// cylindrical coordinates (rho, z >= 0) of the body frame closer than rd to the solid spheroid x^2/A^2 + z^2/C^2 <= 1?
+// Inside: yes.  Outside: the closest point of the ellipse is (A^2 rho/(t + A^2), C^2 z/(t + C^2)) for the root t of
+// F(t) = (A rho/(t + A^2))^2 + (C z/(t + C^2))^2 - 1, which is convex and decreasing: SIX Newton steps from the lower bound
+// t0 = max(A rho - A^2, C z - C^2) approach it monotonically (fp32-converged after five); only + x / on both sides.
+static inline bool near_spheroid(float A, float Cc, float rd2, float rho, float z) {
+  const float qa = rho / A, qc = z / Cc;
+  if (fmaf(qa, qa, qc * qc) <= 1.0f) return true;
+  const float A2 = A * A, C2 = Cc * Cc, ar = A * rho, cz = Cc * z;
+  float t = ar - A2;
+  const float t1 = cz - C2;
+  if (t1 > t) t = t1;
+  for (int it = 0; it < 6; ++it) {
+    const float ia = 1.0f / (t + A2), ic = 1.0f / (t + C2);
+    const float ua = ar * ia, uc = cz * ic;
+    const float ua2 = ua * ua, uc2 = uc * uc;
+    const float F = (ua2 + uc2) - 1.0f;
+    const float dF = -2.0f * (ua2 * ia + uc2 * ic);
+    t = t - F / dF;
+  }
+  const float ex = rho - (A2 * rho) / (t + A2), ez = z - (C2 * z) / (t + C2);
+  return fmaf(ex, ex, ez * ez) < rd2;
+}
+
 // Depletant (sphere radius rd, centre at d relative to the colloid centre) vs colloid with
-// body axis a.  R-S14 (strict <), R-S16 (half-ball), R-S17 (spherodisk).
+// body axis a.  R-S14 (strict <), R-S16 (half-ball), R-S17 (spherodisk), R-N2 (ellipsoid).
 static inline bool dep_overlap(const Geo& g, V3 d, V3 a) {
   const float d2 = dot3(d, d);
   if (!(d2 < g.Rins2)) return false;          // circumsphere (+) depletant
   if (g.shape == SH_SPHERE) return true;
   const float bz = dot3(d, a);
+  if (g.shape == SH_ELLIPSOID) {
+    const V3 p = V3{d.x - bz * a.x, d.y - bz * a.y, d.z - bz * a.z};
+    return near_spheroid(g.adisk, g.sdisk, g.rd2, sqrtf(dot3(p, p)), fabsf(bz));
+  }
   if (g.shape == SH_HALFBALL) {
     if (bz <= 0.0f) return true;              // below the flat face: inside ball radius Rh+rd
     const V3 p = V3{d.x - bz * a.x, d.y - bz * a.y, d.z - bz * a.z};
@@ -190,6 +218,14 @@ static inline V3 support(const Geo& g, V3 a, V3 n) {
     const float l = sqrtf(dot3(p, p));
     if (!(l > 0.0f)) return V3{0.0f, 0.0f, 0.0f};
     return p * (g.Rh / l);
+  }
+  if (g.shape == SH_ELLIPSOID) {               // (A^2 n_perp + C^2 n_par a) / sqrt(A^2 |n_perp|^2 + C^2 n_par^2)
+    const V3 p = V3{n.x - nz * a.x, n.y - nz * a.y, n.z - nz * a.z};
+    const float A2 = g.adisk * g.adisk, C2 = g.sdisk * g.sdisk;
+    const float den = sqrtf(A2 * dot3(p, p) + C2 * (nz * nz));
+    if (!(den > 0.0f)) return V3{0.0f, 0.0f, 0.0f};
+    const float wa = A2 / den, wc = (C2 * nz) / den;
+    return V3{wa * p.x + wc * a.x, wa * p.y + wc * a.y, wa * p.z + wc * a.z};
   }
   // spherodisk: disk rim point + rounding sphere
   const V3 p = V3{n.x - nz * a.x, n.y - nz * a.y, n.z - nz * a.z};
@@ -392,7 +428,7 @@ struct Shell { float Rin, Rin3, dR3; };
 static inline Shell make_shell(const Geo& g, float d_max, uint32_t flags) {
   float rin = g.Rins;
   if (g.shape == SH_HALFBALL) rin = g.rd;
-  else if (g.shape == SH_SPHERODISK) rin = g.sdisk + g.rd;
+  else if (g.shape == SH_SPHERODISK || g.shape == SH_ELLIPSOID) rin = g.sdisk + g.rd;   // rounding radius / polar semi-axis
   Shell sh;
   sh.Rin = rin - 1.7320508f * d_max;
   if (sh.Rin < 0.0f) sh.Rin = 0.0f;

@@ -32,6 +32,8 @@ def _gold(key):
 HB = dict(shape="halfball", sigma_c=1.0, sigma_d=0.2, box_L=20.0, d_max_cap=0.1)
 SD = dict(shape="spherodisk", sigma_c=1.0, sigma_d=0.15, box_L=20.0, d_max_cap=0.1, disk_a=0.4, disk_s=0.1)
 SP = dict(shape="sphere", sigma_c=1.0, sigma_d=0.2, box_L=20.0, d_max_cap=0.1)
+# the paper's discoids (L228): oblate ellipsoids a = b = 0.5, c = 0.25, depletant radius 0.25 (disk_a = A, disk_s = C)
+EL = dict(shape="ellipsoid", sigma_c=1.0, sigma_d=0.5, box_L=20.0, d_max_cap=0.1, disk_a=0.5, disk_s=0.25)
 
 
 def rand_quats(n, rng):
@@ -80,6 +82,16 @@ def shape_cloud(params, n, rng):
         face = np.stack([rad * np.cos(ang), rad * np.sin(ang), np.zeros(n)], -1)
         rim = np.stack([R * np.cos(ang), R * np.sin(ang), np.zeros(n)], -1)
         return np.concatenate([vol, dome, face, rim])
+    if params["shape"] == "ellipsoid":
+        A, Cc = params["disk_a"], params["disk_s"]
+        v = rng.standard_normal((n, 3))
+        v /= np.linalg.norm(v, axis=1, keepdims=True)
+        sc = np.array([A, A, Cc])
+        # surface points (denser near the equator, where curvature is highest) and interior points
+        th = rng.random(n) * np.pi
+        ph = rng.random(n) * 2 * np.pi
+        eq = np.stack([A * np.sin(th) * np.cos(ph), A * np.sin(th) * np.sin(ph), Cc * np.cos(th)], -1)
+        return np.concatenate([v * sc, eq, v * sc * rng.random((n, 1)) ** (1 / 3)])
     a, s = params["disk_a"], params["disk_s"]
     ang, rad = rng.random(n) * 2 * np.pi, a * np.sqrt(rng.random(n))
     disk = np.stack([rad * np.cos(ang), rad * np.sin(ang), np.zeros(n)], -1)
@@ -103,6 +115,43 @@ def test_dilated_volume_steiner(olib, params, key):
     assert abs(frac - want) < 4.5 * math.sqrt(want * (1 - want) / n) + 2e-5
 
 
+def _spheroid_steiner_volume(A, Cc, r):
+    """Volume of the oblate spheroid (A, A, Cc) dilated by a ball of radius r: V + S r + M r^2 + 4 pi r^3 / 3 (Steiner),
+    with the surface area S and the integrated mean curvature M = 2 pi x (mean width) by quadrature of their closed-form
+    integrands: surface of revolution (A sin t, Cc cos t); support function h(t) = sqrt(A^2 sin^2 t + Cc^2 cos^2 t)."""
+    from scipy.integrate import quad
+    V = 4.0 * math.pi * A * A * Cc / 3.0
+    S = quad(lambda t: 2 * math.pi * A * math.sin(t) * math.sqrt((A * math.cos(t)) ** 2 + (Cc * math.sin(t)) ** 2), 0, math.pi)[0]
+    M = 2 * math.pi * quad(lambda t: math.sqrt((A * math.sin(t)) ** 2 + (Cc * math.cos(t)) ** 2) * math.sin(t), 0, math.pi)[0]
+    return V + S * r + M * r * r + 4.0 * math.pi * r ** 3 / 3.0
+
+
+def test_steiner_formula_on_spheres_and_dilated_volume_ellipsoid(olib):
+    """R-N2: fraction of insertion-ball samples that overlap the ellipsoid = Steiner volume / ball volume (4.5 sigma at 1e6).
+    The quadrature itself is checked on the sphere (A = Cc), where the Steiner sum is 4 pi (A + r)^3 / 3."""
+    assert abs(_spheroid_steiner_volume(0.5, 0.5, 0.25) / (4 * math.pi * 0.75 ** 3 / 3) - 1) < 1e-9
+    n = 1000000
+    R = 0.5 * (EL["sigma_c"] + EL["sigma_d"])
+    d = np.zeros((n, 3), np.float32)
+    olib.oracle_ball_samples(3, 1, 0, 79, n, R, d.ctypes.data)
+    for seed in (5, 6):
+        q = rand_quats(1, np.random.default_rng(seed))[0]
+        frac = dep_overlap(EL, q, d).mean()
+        want = _spheroid_steiner_volume(EL["disk_a"], EL["disk_s"], 0.5 * EL["sigma_d"]) / (4 * math.pi * R ** 3 / 3)
+        assert abs(frac - want) < 4.5 * math.sqrt(want * (1 - want) / n) + 2e-5, (frac, want)
+
+
+def test_pair_overlap_closed_forms_ellipsoid():
+    """Coaxial spheroids overlap iff |dz| < 2 C; coplanar ones (same axis, separation in the equatorial plane) iff the
+    distance is < 2 A; an edge-on spheroid above a flat one (axes perpendicular) iff the gap is < A + C."""
+    A, Cc = EL["disk_a"], EL["disk_s"]
+    z, x = quat_from_axis([0, 0, 1]), quat_from_axis([1, 0, 0])
+    for gap in (-0.05, -0.002, 0.002, 0.05):
+        assert pair_overlap(EL, [0, 0, 2 * Cc + gap], z, z)[0] == (gap < 0)
+        assert pair_overlap(EL, [2 * A + gap, 0, 0], z, z)[0] == (gap < 0)
+        assert pair_overlap(EL, [0, 0, A + Cc + gap], z, x)[0] == (gap < 0)
+
+
 def test_dilated_volume_sphere(olib):
     n = 100000
     d = np.zeros((n, 3), np.float32)
@@ -116,7 +165,7 @@ def test_spherodisk_volume_formula():
     assert abs(workloads.spherodisk_volume(0.4, 0.1) - _gold("spherodisk_volume")) < 1e-6
 
 
-@pytest.mark.parametrize("params", [HB, SD])
+@pytest.mark.parametrize("params", [HB, SD, EL])
 def test_dep_overlap_vs_point_cloud(params):
     """Predicate == (distance from the depletant centre to the solid < r_d), by brute force."""
     rng = np.random.default_rng(11)
@@ -137,7 +186,7 @@ def test_dep_overlap_vs_point_cloud(params):
 
 
 # ----------------------------------------------------------------------------------- support function
-@pytest.mark.parametrize("params", [HB, SD])
+@pytest.mark.parametrize("params", [HB, SD, EL])
 def test_support_is_argmax_over_cloud(olib, params):
     rng = np.random.default_rng(12)
     cloud = shape_cloud(params, 100000, rng)
@@ -161,6 +210,8 @@ def test_support_is_argmax_over_cloud(olib, params):
         olib.oracle_support(C.byref(p), ident.ctypes.data, nv.ctypes.data, out.ctypes.data)
         if params["shape"] == "halfball":
             exp = {(0, 0, 1): 0.0, (0, 0, -1): 0.5, (1, 0, 0): 0.5}[tuple(n)]
+        elif params["shape"] == "ellipsoid":
+            exp = {(0, 0, 1): 0.25, (0, 0, -1): 0.25, (1, 0, 0): 0.5}[tuple(n)]
         else:
             exp = {(0, 0, 1): 0.1, (0, 0, -1): 0.1, (1, 0, 0): 0.5}[tuple(n)]
         assert abs(float(out @ nv) - exp) < 1e-6
@@ -242,6 +293,10 @@ def _gauge(params):
     if params["shape"] == "halfball":
         R = 0.5 * params["sigma_c"]
         return lambda b: max(np.linalg.norm(b) - R, b[2])
+    if params["shape"] == "ellipsoid":
+        A, Cc = params["disk_a"], params["disk_s"]
+        # convex, <= 0 inside, and at least as large as the signed distance scaled by 1/A near the surface
+        return lambda b: Cc * (math.sqrt((b[0] * b[0] + b[1] * b[1]) / (A * A) + b[2] * b[2] / (Cc * Cc)) - 1.0)
     a, s = params["disk_a"], params["disk_s"]
 
     def g(b):
@@ -269,7 +324,7 @@ def _deepest_common_point(params, rho, qA, qB):
     return best
 
 
-@pytest.mark.parametrize("params", [HB, SD])
+@pytest.mark.parametrize("params", [HB, SD, EL])
 def test_pair_overlap_vs_convex_program(params):
     """Random poses inside the circumsphere range: MPR's verdict == sign of the fp64 convex program,
     outside a contact band."""

@@ -30,7 +30,7 @@ def spherodisk_volume(a: float, s: float) -> float:
 class Config:
     name: str
     N: int
-    shape: str            # "sphere" | "halfball" | "spherodisk"
+    shape: str            # "sphere" | "halfball" | "spherodisk" | "ellipsoid"
     phi_c: float          # colloid packing fraction
     q: float              # sigma_d / sigma_c
     phi_d_r: tuple        # reservoir packing fraction(s) of the depletants
@@ -50,6 +50,8 @@ class Config:
             return SPHERE_VOL * self.sigma_c ** 3
         if self.shape == "halfball":
             return HALFBALL_VOL * self.sigma_c ** 3
+        if self.shape == "ellipsoid":          # oblate spheroid, semi-axes (disk_a, disk_a, disk_s)
+            return 4.0 * math.pi * self.disk_a ** 2 * self.disk_s / 3.0
         return spherodisk_volume(self.disk_a, self.disk_s)
 
     @property
@@ -78,6 +80,10 @@ _CONFIGS = {
     "C3": Config("C3", 1048576, "sphere", 0.25, 0.05, (0.30,), 0.05, 0.0, 0, 200, "rsa"),
     "C4": Config("C4", 32768, "halfball", 0.20, 0.20, (0.25,), 0.1, 0.1, 0, 500, "sc"),
     "C5": Config("C5", 32768, "spherodisk", 0.15, 0.15, (0.35,), 0.1, 0.1, 4, 500, "sc", disk_a=0.4, disk_s=0.1),
+    # SURVEY 8(f) NEXT-2, not a BASELINE.json config: the paper's own discoids (oblate ellipsoids
+    # a = b = 0.5, c = 0.25, depletant radius 0.25, phi_p^r = 0.40, n_trial >~ 10), here 32^3 of them at phi_c = 0.10
+    # (the paper's 500 at phi_c = 0.01 would leave every neighbourhood empty) with C4's step sizes
+    "C6": Config("C6", 32768, "ellipsoid", 0.10, 0.50, (0.40,), 0.1, 0.1, 10, 200, "sc", disk_a=0.5, disk_s=0.25),
 }
 
 
@@ -178,7 +184,7 @@ def generate(cfg: Config):
         pos = _sc_sites(n, L)
         spacing = L / n
         quat = _random_quats(N, rng)
-        if cfg.shape == "halfball":
+        if cfg.shape in ("halfball", "ellipsoid"):
             if spacing < cfg.sigma_c * 1.0001:
                 raise ValueError("circumspheres of the lattice overlap")
         elif cfg.shape == "spherodisk":
