@@ -34,7 +34,9 @@ typedef struct hpmc_ctx hpmc_ctx; /* opaque, library-owned */
 typedef enum {
   HPMC_SPHERE = 0,     /* sphere of diameter sigma_c */
   HPMC_HALFBALL = 1,   /* {x: |x| <= sigma_c/2, x.z_body <= 0}: flat face through the pose centre, outward normal +z_body */
-  HPMC_SPHERODISK = 2  /* Minkowski sum of a flat disk (radius disk_a, normal z_body) and a ball (radius disk_s) */
+  HPMC_SPHERODISK = 2, /* Minkowski sum of a flat disk (radius disk_a, normal z_body) and a ball (radius disk_s) */
+  HPMC_ELLIPSOID = 3   /* oblate spheroid, semi-axes (disk_a, disk_a, disk_s), disk_a >= disk_s > 0, short axis z_body: the paper's
+                          discoids (reading R-N2); sigma_c must equal 2 disk_a */
 } hpmc_shape;
 
 typedef enum {
@@ -54,8 +56,9 @@ typedef enum {
 typedef struct {
   int32_t shape;       /* hpmc_shape */
   float sigma_c;       /* circumsphere diameter d_colloid: sphere diameter, 2 R_halfball, 2 (disk_a + disk_s) */
-  float disk_a;        /* spherodisk only: disk radius a >= 0 */
-  float disk_s;        /* spherodisk only: rounding radius s >= 0; sigma_c must equal 2 (a + s), else HPMC_E_BADARG */
+  float disk_a;        /* spherodisk: disk radius a >= 0; ellipsoid: equatorial semi-axis */
+  float disk_s;        /* spherodisk: rounding radius s >= 0, sigma_c must equal 2 (a + s); ellipsoid: polar semi-axis,
+                          sigma_c must equal 2 disk_a; else HPMC_E_BADARG */
   float sigma_d;       /* depletant diameter d_depletant (>= 0) */
   float box_L;         /* edge of the cubic periodic box */
   float d_max_cap;     /* largest d_max any later sweep will use; fixes the cell width

@@ -10,7 +10,7 @@
 
 namespace hpmc {
 
-enum : int { SH_SPHERE = 0, SH_HALFBALL = 1, SH_SPHERODISK = 2 };
+enum : int { SH_SPHERE = 0, SH_HALFBALL = 1, SH_SPHERODISK = 2, SH_ELLIPSOID = 3 };
 
 struct Geo {              // derived constants, computed once on the host in fp32
   float L, halfL, w;      // box edge, L/2, cell width
@@ -20,7 +20,7 @@ struct Geo {              // derived constants, computed once on the host in fp3
   float rcut2;            // neighbour pre-filter radius squared
   float rd, rd2;          // depletant radius
   float Rh, cen;          // half-ball radius and interior-point offset 3 Rh / 8
-  float adisk, sdisk, rs2;
+  float adisk, sdisk, rs2;  // spherodisk: disk radius, rounding radius, (s + r_d)^2; ellipsoid: semi-axes A >= C in adisk, sdisk
 };
 
 struct V3 { float x, y, z; };
@@ -57,6 +57,30 @@ __device__ __forceinline__ Q4 rotate_cayley(Q4 q, V3 v) {
   return Q4{__fdiv_rn(pw, n), __fdiv_rn(px, n), __fdiv_rn(py, n), __fdiv_rn(pz, n)};
 }
 
+// R-N2 (oblate spheroid x^2/A^2 + z^2/C^2 <= 1 in cylindrical body coordinates, the paper's discoids L228): is the point
+// (rho, z >= 0) closer than r_d to the solid?  Inside: yes.  Outside: the closest point of the ellipse is
+// (A^2 rho/(t + A^2), C^2 z/(t + C^2)) for the root t of F(t) = (A rho/(t + A^2))^2 + (C z/(t + C^2))^2 - 1 (convex,
+// decreasing); six Newton steps from the lower bound max(A rho - A^2, C z - C^2), IEEE division throughout.
+__device__ __forceinline__ bool near_spheroid(float A, float Cc, float rd2, float rho, float z) {
+  const float qa = __fdiv_rn(rho, A), qc = __fdiv_rn(z, Cc);
+  if (fmaf(qa, qa, qc * qc) <= 1.0f) return true;
+  const float A2 = A * A, C2 = Cc * Cc, ar = A * rho, cz = Cc * z;
+  float t = ar - A2;
+  const float t1 = cz - C2;
+  if (t1 > t) t = t1;
+#pragma unroll 1
+  for (int it = 0; it < 6; ++it) {
+    const float ia = __fdiv_rn(1.0f, t + A2), ic = __fdiv_rn(1.0f, t + C2);
+    const float ua = ar * ia, uc = cz * ic;
+    const float ua2 = ua * ua, uc2 = uc * uc;
+    const float F = (ua2 + uc2) - 1.0f;
+    const float dF = -2.0f * (ua2 * ia + uc2 * ic);
+    t = t - __fdiv_rn(F, dF);
+  }
+  const float ex = rho - __fdiv_rn(A2 * rho, t + A2), ez = z - __fdiv_rn(C2 * z, t + C2);
+  return fmaf(ex, ex, ez * ez) < rd2;
+}
+
 // Does a depletant centred at d (relative to the colloid centre) overlap the colloid with body axis a?
 template <int SHAPE>
 __device__ __forceinline__ bool dep_overlap(const Geo& g, V3 d, V3 a) {
@@ -64,6 +88,10 @@ __device__ __forceinline__ bool dep_overlap(const Geo& g, V3 d, V3 a) {
   if (!(d2 < g.Rins2)) return false;
   if (SHAPE == SH_SPHERE) return true;
   const float bz = dot3(d, a);
+  if (SHAPE == SH_ELLIPSOID) {
+    const V3 p = V3{d.x - bz * a.x, d.y - bz * a.y, d.z - bz * a.z};
+    return near_spheroid(g.adisk, g.sdisk, g.rd2, __fsqrt_rn(dot3(p, p)), fabsf(bz));
+  }
   if (SHAPE == SH_HALFBALL) {
     if (bz <= 0.0f) return true;
     const V3 p = V3{d.x - bz * a.x, d.y - bz * a.y, d.z - bz * a.z};
@@ -92,6 +120,14 @@ __device__ __forceinline__ V3 support(const Geo& g, V3 a, V3 n) {
     const float l = __fsqrt_rn(dot3(p, p));
     if (!(l > 0.0f)) return V3{0.0f, 0.0f, 0.0f};
     return p * __fdiv_rn(g.Rh, l);
+  }
+  if (SHAPE == SH_ELLIPSOID) {               // (A^2 n_perp + C^2 n_par a) / sqrt(A^2 |n_perp|^2 + C^2 n_par^2)
+    const V3 p = V3{n.x - nz * a.x, n.y - nz * a.y, n.z - nz * a.z};
+    const float A2 = g.adisk * g.adisk, C2 = g.sdisk * g.sdisk;
+    const float den = __fsqrt_rn(A2 * dot3(p, p) + C2 * (nz * nz));
+    if (!(den > 0.0f)) return V3{0.0f, 0.0f, 0.0f};
+    const float wa = __fdiv_rn(A2, den), wc = __fdiv_rn(C2 * nz, den);
+    return V3{wa * p.x + wc * a.x, wa * p.y + wc * a.y, wa * p.z + wc * a.z};
   }
   const V3 p = V3{n.x - nz * a.x, n.y - nz * a.y, n.z - nz * a.z};
   const float l = __fsqrt_rn(dot3(p, p));
