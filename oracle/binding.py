@@ -25,7 +25,7 @@ COUNTER_NAMES = (
     "philox_blocks",
 )
 
-SHAPES = {"sphere": 0, "halfball": 1, "spherodisk": 2, "ellipsoid": 3}
+SHAPES = {"sphere": 0, "halfball": 1, "spherodisk": 2, "ellipsoid": 3, "tetrahedron": 4}
 FLAG_SHELL, FLAG_ROSENBLUTH, FLAG_TEST_LITERAL_CORE = 1, 2, 0x100
 
 

@@ -118,7 +118,7 @@ static inline Q4 rotate_cayley(Q4 q, V3 v) {
 }
 
 // ----------------------------------------------------------------------------- shapes
-enum { SH_SPHERE = 0, SH_HALFBALL = 1, SH_SPHERODISK = 2, SH_ELLIPSOID = 3 };
+enum { SH_SPHERE = 0, SH_HALFBALL = 1, SH_SPHERODISK = 2, SH_ELLIPSOID = 3, SH_TETRAHEDRON = 4 };
 
 struct Geo {                 // derived fp32 constants, R-0
   int shape;
@@ -154,6 +154,74 @@ static Geo make_geo(int shape, float sigma_c, float disk_a, float disk_s, float 
   return g;
 }
 
+// Orientation as the shape tests need it: the body z axis (x, y, z; w unused) for the bodies of revolution (R-S19), the
+// whole unit quaternion (w, x, y, z stored as x = q.w, y = q.x, z = q.y, w = q.z) for the tetrahedron.
+struct Ori { float x, y, z, w; };
+static inline Ori ori_of(const Geo& g, Q4 q) {
+  if (g.shape == SH_TETRAHEDRON) return Ori{q.w, q.x, q.y, q.z};
+  const V3 a = quat_axis(q);
+  return Ori{a.x, a.y, a.z, 0.0f};
+}
+static inline V3 axis_of(Ori o) { return V3{o.x, o.y, o.z}; }
+
+// R-N2b (Fig. 1 L21 shows tetrahedra): regular tetrahedron with circumradius Rh = sigma_c / 2, body-frame
+// vertices s u_i, s = Rh 0.57735026f, u_0 = (1,1,1), u_1 = (1,-1,-1), u_2 = (-1,1,-1), u_3 = (-1,-1,1); the face opposite
+// vertex i lies in the plane u_i . x = -s.  Body axes = columns of the rotation matrix of q (the formula of R-S19 for all three).
+struct Frame { V3 ex, ey, ez; };
+static inline Frame frame_of(Ori o) {
+  const float w = o.x, x = o.y, y = o.z, z = o.w;
+  Frame f;
+  f.ex = V3{1.0f - 2.0f * (y * y + z * z), 2.0f * (x * y + w * z), 2.0f * (x * z - w * y)};
+  f.ey = V3{2.0f * (x * y - w * z), 1.0f - 2.0f * (x * x + z * z), 2.0f * (y * z + w * x)};
+  f.ez = V3{2.0f * (x * z + w * y), 2.0f * (y * z - w * x), 1.0f - 2.0f * (x * x + y * y)};
+  return f;
+}
+static const float TET_U[4][3] = {{1.0f, 1.0f, 1.0f}, {1.0f, -1.0f, -1.0f}, {-1.0f, 1.0f, -1.0f}, {-1.0f, -1.0f, 1.0f}};
+
+// squared distance from p to the triangle (a, b, c): closest-point regions by barycentric signs (Ericson, Real-Time
+// Collision Detection 5.1.5), only + x /
+static inline float tri_dist2(V3 p, V3 a, V3 b, V3 c) {
+  const V3 ab = b - a, ac = c - a, ap = p - a;
+  const float d1 = dot3(ab, ap), d2 = dot3(ac, ap);
+  if (d1 <= 0.0f && d2 <= 0.0f) return dot3(ap, ap);
+  const V3 bp = p - b;
+  const float d3 = dot3(ab, bp), d4 = dot3(ac, bp);
+  if (d3 >= 0.0f && d4 <= d3) return dot3(bp, bp);
+  const float vc = d1 * d4 - d3 * d2;
+  if (vc <= 0.0f && d1 >= 0.0f && d3 <= 0.0f) { const float v = d1 / (d1 - d3); const V3 e = ap - ab * v; return dot3(e, e); }
+  const V3 cp = p - c;
+  const float d5 = dot3(ab, cp), d6 = dot3(ac, cp);
+  if (d6 >= 0.0f && d5 <= d6) return dot3(cp, cp);
+  const float vb = d5 * d2 - d1 * d6;
+  if (vb <= 0.0f && d2 >= 0.0f && d6 <= 0.0f) { const float w = d2 / (d2 - d6); const V3 e = ap - ac * w; return dot3(e, e); }
+  const float va = d3 * d6 - d5 * d4;
+  if (va <= 0.0f && (d4 - d3) >= 0.0f && (d5 - d6) >= 0.0f) {
+    const float w = (d4 - d3) / ((d4 - d3) + (d5 - d6));
+    const V3 e = bp - (c - b) * w;
+    return dot3(e, e);
+  }
+  const float den = 1.0f / (va + vb + vc);
+  const float v = vb * den, w = vc * den;
+  const V3 e = ap - (ab * v + ac * w);
+  return dot3(e, e);
+}
+// depletant centre at body-frame point b vs the tetrahedron: inside, or closer than rd to a face it lies in front of
+static inline bool near_tetrahedron(float s, float rd2, V3 b) {
+  V3 v[4];
+  for (int i = 0; i < 4; ++i) v[i] = V3{s * TET_U[i][0], s * TET_U[i][1], s * TET_U[i][2]};
+  bool inside = true;
+  float best = 3.0e38f;
+  for (int i = 0; i < 4; ++i) {
+    const float h = (TET_U[i][0] * b.x + TET_U[i][1] * b.y) + TET_U[i][2] * b.z;
+    if (h < -s) {                                  // in front of the face opposite vertex i
+      inside = false;
+      const float d2 = tri_dist2(b, v[(i + 1) & 3], v[(i + 2) & 3], v[(i + 3) & 3]);
+      if (d2 < best) best = d2;
+    }
+  }
+  return inside || best < rd2;
+}
+
 // R-N2 (the paper's discoids are oblate ellipsoids a = b = 0.5, c = 0.25, L228): is the point at
 // cylindrical coordinates (rho, z >= 0) of the body frame closer than rd to the solid spheroid x^2/A^2 + z^2/C^2 <= 1?
 // Inside: yes.  Outside: the closest point of the ellipse is (A^2 rho/(t + A^2), C^2 z/(t + C^2)) for the root t of
@@ -180,10 +248,15 @@ static inline bool near_spheroid(float A, float Cc, float rd2, float rho, float 
 
 // Depletant (sphere radius rd, centre at d relative to the colloid centre) vs colloid with
 // body axis a.  R-S14 (strict <), R-S16 (half-ball), R-S17 (spherodisk), R-N2 (ellipsoid).
-static inline bool dep_overlap(const Geo& g, V3 d, V3 a) {
+static inline bool dep_overlap(const Geo& g, V3 d, Ori o) {
   const float d2 = dot3(d, d);
   if (!(d2 < g.Rins2)) return false;          // circumsphere (+) depletant
   if (g.shape == SH_SPHERE) return true;
+  if (g.shape == SH_TETRAHEDRON) {
+    const Frame f = frame_of(o);
+    return near_tetrahedron(g.Rh * 0.57735026f, g.rd2, V3{dot3(d, f.ex), dot3(d, f.ey), dot3(d, f.ez)});
+  }
+  const V3 a = axis_of(o);
   const float bz = dot3(d, a);
   if (g.shape == SH_ELLIPSOID) {
     const V3 p = V3{d.x - bz * a.x, d.y - bz * a.y, d.z - bz * a.z};
@@ -206,7 +279,20 @@ static inline bool dep_overlap(const Geo& g, V3 d, V3 a) {
 }
 
 // Support point of the shape with body axis a, centred at the origin, in direction n. R-S18.
-static inline V3 support(const Geo& g, V3 a, V3 n) {
+static inline V3 support(const Geo& g, Ori o, V3 n) {
+  if (g.shape == SH_TETRAHEDRON) {               // the vertex with the largest projection (first one on ties)
+    const Frame f = frame_of(o);
+    const V3 nb = V3{dot3(n, f.ex), dot3(n, f.ey), dot3(n, f.ez)};
+    int best = 0;
+    float hb = (TET_U[0][0] * nb.x + TET_U[0][1] * nb.y) + TET_U[0][2] * nb.z;
+    for (int i = 1; i < 4; ++i) {
+      const float h = (TET_U[i][0] * nb.x + TET_U[i][1] * nb.y) + TET_U[i][2] * nb.z;
+      if (h > hb) { hb = h; best = i; }
+    }
+    const float s = g.Rh * 0.57735026f;
+    return (f.ex * (s * TET_U[best][0]) + f.ey * (s * TET_U[best][1])) + f.ez * (s * TET_U[best][2]);
+  }
+  const V3 a = axis_of(o);
   const float nz = dot3(n, a);
   if (g.shape == SH_HALFBALL) {
     if (nz <= 0.0f) {
@@ -241,7 +327,7 @@ static const int MPR_MAXIT = 48;
 static const float MPR_TOL = 1e-5f;
 
 // Support of the Minkowski difference B - A in direction n (A at origin, B at rho).
-static inline V3 support_diff(const Geo& g, V3 rho, V3 aA, V3 aB, V3 n) {
+static inline V3 support_diff(const Geo& g, V3 rho, Ori aA, Ori aB, V3 n) {
   const V3 sb = support(g, aB, n);
   const V3 sa = support(g, aA, neg(n));
   return (sb + rho) - sa;
@@ -250,11 +336,11 @@ static inline V3 support_diff(const Geo& g, V3 rho, V3 aA, V3 aB, V3 n) {
 // Minkowski-portal-refinement (XenoCollide, G. Snethen 2008) boolean overlap test on the
 // full convex shapes.  R-S18.  Returns true if overlapping.  Contact band (|gap| < MPR_TOL)
 // counts as not overlapping; iteration cap counts as overlapping.
-static bool mpr_overlap(const Geo& g, V3 rho, V3 aA, V3 aB) {
+static bool mpr_overlap(const Geo& g, V3 rho, Ori aA, Ori aB) {
   V3 cA = V3{0.0f, 0.0f, 0.0f}, cB = rho;
   if (g.shape == SH_HALFBALL) {
-    cA = neg(aA * g.cen);
-    cB = rho - aB * g.cen;
+    cA = neg(axis_of(aA) * g.cen);
+    cB = rho - axis_of(aB) * g.cen;
   }
   V3 v0 = cB - cA;
   if (v0.x == 0.0f && v0.y == 0.0f && v0.z == 0.0f) v0 = V3{1e-5f, 0.0f, 0.0f};
@@ -297,7 +383,7 @@ static bool mpr_overlap(const Geo& g, V3 rho, V3 aA, V3 aB) {
 }
 
 // Hard overlap of colloid A (origin, axis aA) with colloid B (at rho, axis aB).  Eq. 5 L80.
-static inline bool pair_overlap(const Geo& g, V3 rho, V3 aA, V3 aB) {
+static inline bool pair_overlap(const Geo& g, V3 rho, Ori aA, Ori aB) {
   const float r2 = dot3(rho, rho);
   if (!(r2 < g.dcirc2)) return false;          // circumsphere pre-test (exact test for spheres)
   if (g.shape == SH_SPHERE) return true;
@@ -429,6 +515,7 @@ static inline Shell make_shell(const Geo& g, float d_max, uint32_t flags) {
   float rin = g.Rins;
   if (g.shape == SH_HALFBALL) rin = g.rd;
   else if (g.shape == SH_SPHERODISK || g.shape == SH_ELLIPSOID) rin = g.sdisk + g.rd;   // rounding radius / polar semi-axis
+  else if (g.shape == SH_TETRAHEDRON) rin = g.Rh * 0.33333334f + g.rd;                   // inradius of the regular tetrahedron
   Shell sh;
   sh.Rin = rin - 1.7320508f * d_max;
   if (sh.Rin < 0.0f) sh.Rin = 0.0f;
@@ -463,7 +550,7 @@ static inline V3 shell_sample(uint32_t seed, uint32_t step, uint32_t purpose, ui
   return V3{radius, 0.0f, 0.0f};
 }
 
-struct Nbr { V3 rho; V3 axis; };
+struct Nbr { V3 rho; Ori axis; };
 
 // Steps 3.4 - 3.8 of the move: neighbourhood, hard overlap, depletants.
 // i = moved colloid, own = its cell, (r0,q0) old pose, (r1,q1) new pose (already wrapped).
@@ -483,11 +570,11 @@ static int evaluate_move(const Ctx& c, uint32_t seed, uint32_t step, uint32_t co
           if (j == i) continue;
           const V3 rho = minimg(g, load_r(c, j), r1);
           if (!(dot3(rho, rho) < g.rcut2)) continue;
-          nb.push_back(Nbr{rho, quat_axis(load_q(c, j))});
+          nb.push_back(Nbr{rho, ori_of(g, load_q(c, j))});
         }
       }
   const V3 rho_old = minimg(g, r0, r1);
-  const V3 a_old = quat_axis(q0), a_new = quat_axis(q1);
+  const Ori a_old = ori_of(g, q0), a_new = ori_of(g, q1);
 
   // 3.5 hard overlap of the new pose with any neighbour (Eq. 5's min(1, e^{-beta dH_cc}), L80)
   for (const Nbr& n : nb)
@@ -836,7 +923,7 @@ int oracle_free_volume(void* h, uint32_t seed, uint32_t step, int64_t n, uint64_
           const int64_t cj = ((int64_t)jz * nc + jy) * nc + jx;
           for (uint32_t t = c->cell_start[(size_t)cj]; t < c->cell_start[(size_t)cj + 1]; ++t) {
             const int64_t j = c->cell_pid[t];
-            if (dep_overlap(g, minimg(g, p, load_r(*c, j)), quat_axis(load_q(*c, j)))) { is_free = false; break; }
+            if (dep_overlap(g, minimg(g, p, load_r(*c, j)), ori_of(g, load_q(*c, j)))) { is_free = false; break; }
           }
         }
     cnt += is_free ? 1u : 0u;
@@ -863,7 +950,7 @@ int64_t oracle_count_overlaps(void* h, int32_t both_ways) {
   }
   int64_t count = 0;
   for (int64_t i = 0; i < c->N; ++i) {
-    const V3 ri = load_r(*c, i); const V3 ai = quat_axis(load_q(*c, i));
+    const V3 ri = load_r(*c, i); const Ori ai = ori_of(g, load_q(*c, i));
     const int ix = ax(ri.x), iy = ax(ri.y), iz = ax(ri.z);
     std::vector<int64_t> seen;
     for (int dz = -1; dz <= 1; ++dz) for (int dy = -1; dy <= 1; ++dy) for (int dx = -1; dx <= 1; ++dx) {
@@ -872,7 +959,7 @@ int64_t oracle_count_overlaps(void* h, int32_t both_ways) {
         if ((int64_t)j <= i) continue;
         if (std::find(seen.begin(), seen.end(), (int64_t)j) != seen.end()) continue;   // n < 3 aliasing
         seen.push_back(j);
-        const V3 aj = quat_axis(load_q(*c, j));
+        const Ori aj = ori_of(g, load_q(*c, j));
         bool o = pair_overlap(g, minimg(g, load_r(*c, j), ri), ai, aj);
         if (o && both_ways) o = pair_overlap(g, minimg(g, ri, load_r(*c, j)), aj, ai);
         if (o) ++count;
@@ -934,7 +1021,7 @@ void oracle_ball_samples(uint32_t seed, uint32_t step, uint32_t colour, uint32_t
 // depletant-vs-colloid predicate for n displacement vectors d (depletant centre - colloid centre)
 void oracle_dep_overlap(const oracle_params* p, const float* quat4, const float* d3, int64_t n, uint8_t* out) {
   const Geo g = make_geo(p->shape, p->sigma_c, p->disk_a, p->disk_s, p->sigma_d, p->box_L, p->d_max_cap);
-  const V3 a = quat_axis(Q4{quat4[0], quat4[1], quat4[2], quat4[3]});
+  const Ori a = ori_of(g, Q4{quat4[0], quat4[1], quat4[2], quat4[3]});
   for (int64_t k = 0; k < n; ++k) out[k] = dep_overlap(g, V3{d3[3 * k], d3[3 * k + 1], d3[3 * k + 2]}, a) ? 1 : 0;
 }
 // colloid-colloid predicate for n pairs: A at origin with qA, B at rho with qB
@@ -942,14 +1029,14 @@ void oracle_pair_overlap(const oracle_params* p, const float* rho3, const float*
                          uint8_t* out) {
   const Geo g = make_geo(p->shape, p->sigma_c, p->disk_a, p->disk_s, p->sigma_d, p->box_L, p->d_max_cap);
   for (int64_t k = 0; k < n; ++k) {
-    const V3 aA = quat_axis(Q4{qA4[4 * k], qA4[4 * k + 1], qA4[4 * k + 2], qA4[4 * k + 3]});
-    const V3 aB = quat_axis(Q4{qB4[4 * k], qB4[4 * k + 1], qB4[4 * k + 2], qB4[4 * k + 3]});
+    const Ori aA = ori_of(g, Q4{qA4[4 * k], qA4[4 * k + 1], qA4[4 * k + 2], qA4[4 * k + 3]});
+    const Ori aB = ori_of(g, Q4{qB4[4 * k], qB4[4 * k + 1], qB4[4 * k + 2], qB4[4 * k + 3]});
     out[k] = pair_overlap(g, V3{rho3[3 * k], rho3[3 * k + 1], rho3[3 * k + 2]}, aA, aB) ? 1 : 0;
   }
 }
 void oracle_support(const oracle_params* p, const float* quat4, const float* n3, float* out3) {
   const Geo g = make_geo(p->shape, p->sigma_c, p->disk_a, p->disk_s, p->sigma_d, p->box_L, p->d_max_cap);
-  const V3 s = support(g, quat_axis(Q4{quat4[0], quat4[1], quat4[2], quat4[3]}), V3{n3[0], n3[1], n3[2]});
+  const V3 s = support(g, ori_of(g, Q4{quat4[0], quat4[1], quat4[2], quat4[3]}), V3{n3[0], n3[1], n3[2]});
   out3[0] = s.x; out3[1] = s.y; out3[2] = s.z;
 }
 void oracle_quat_axis(const float* q, float* out3) {

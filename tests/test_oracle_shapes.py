@@ -33,6 +33,9 @@ HB = dict(shape="halfball", sigma_c=1.0, sigma_d=0.2, box_L=20.0, d_max_cap=0.1)
 SD = dict(shape="spherodisk", sigma_c=1.0, sigma_d=0.15, box_L=20.0, d_max_cap=0.1, disk_a=0.4, disk_s=0.1)
 SP = dict(shape="sphere", sigma_c=1.0, sigma_d=0.2, box_L=20.0, d_max_cap=0.1)
 # the paper's discoids (L228): oblate ellipsoids a = b = 0.5, c = 0.25, depletant radius 0.25 (disk_a = A, disk_s = C)
+# regular tetrahedron with circumradius 0.5 (Fig. 1 L21, reading R-N2b)
+TE = dict(shape="tetrahedron", sigma_c=1.0, sigma_d=0.2, box_L=20.0, d_max_cap=0.1)
+TET_V = (0.5 / math.sqrt(3.0)) * np.array([[1, 1, 1], [1, -1, -1], [-1, 1, -1], [-1, -1, 1]], np.float64)
 EL = dict(shape="ellipsoid", sigma_c=1.0, sigma_d=0.5, box_L=20.0, d_max_cap=0.1, disk_a=0.5, disk_s=0.25)
 
 
@@ -82,6 +85,14 @@ def shape_cloud(params, n, rng):
         face = np.stack([rad * np.cos(ang), rad * np.sin(ang), np.zeros(n)], -1)
         rim = np.stack([R * np.cos(ang), R * np.sin(ang), np.zeros(n)], -1)
         return np.concatenate([vol, dome, face, rim])
+    if params["shape"] == "tetrahedron":
+        def bary(k, m):
+            w = rng.dirichlet(np.ones(k), m)
+            return w
+        vol = bary(4, n) @ TET_V
+        faces = np.concatenate([bary(3, n // 2) @ TET_V[[j for j in range(4) if j != i]] for i in range(4)])
+        edges = np.concatenate([bary(2, n // 8) @ TET_V[[i, j]] for i in range(4) for j in range(i + 1, 4)])
+        return np.concatenate([vol, faces, edges, TET_V])
     if params["shape"] == "ellipsoid":
         A, Cc = params["disk_a"], params["disk_s"]
         v = rng.standard_normal((n, 3))
@@ -141,6 +152,32 @@ def test_steiner_formula_on_spheres_and_dilated_volume_ellipsoid(olib):
         assert abs(frac - want) < 4.5 * math.sqrt(want * (1 - want) / n) + 2e-5, (frac, want)
 
 
+def test_dilated_volume_and_contacts_tetrahedron(olib):
+    """R-N2b.  Steiner volume of the regular tetrahedron (edge a = R sqrt(8/3)) dilated by r: V + S r + M r^2 + 4 pi r^3/3
+    with V = a^3/(6 sqrt 2), S = sqrt(3) a^2, M = (1/2) sum over edges of length x (pi - dihedral) = 3 a (pi - arccos(1/3));
+    the fraction of insertion-ball samples that overlap must match (4.5 sigma at 1e6).  Contacts of two equally oriented
+    tetrahedra (B = A + t): they overlap iff t lies inside A (+) (-A), i.e. |t| < h_A(n) + h_A(-n) along n:
+    2 s along a body axis (edge midpoints: s = R/sqrt 3), R + R/3 along a vertex direction."""
+    R, r = 0.5, 0.1
+    a = R * math.sqrt(8.0 / 3.0)
+    vdil = a ** 3 / (6 * math.sqrt(2)) + math.sqrt(3) * a * a * r + 3 * a * (math.pi - math.acos(1 / 3)) * r * r + 4 * math.pi * r ** 3 / 3
+    n = 1000000
+    d = np.zeros((n, 3), np.float32)
+    olib.oracle_ball_samples(3, 1, 0, 80, n, 0.6, d.ctypes.data)
+    want = vdil / (4 * math.pi * 0.6 ** 3 / 3)
+    for seed in (5, 6):
+        q = rand_quats(1, np.random.default_rng(seed))[0]
+        frac = dep_overlap(TE, q, d).mean()
+        assert abs(frac - want) < 4.5 * math.sqrt(want * (1 - want) / n) + 2e-5, (frac, want)
+    ident = np.array([1, 0, 0, 0], np.float32)
+    s = R / math.sqrt(3)
+    for gap in (-0.05, -0.002, 0.002, 0.05):
+        assert pair_overlap(TE, [2 * s + gap, 0, 0], ident, ident)[0] == (gap < 0)
+        t = (R + R / 3 + gap) / math.sqrt(3)
+        assert pair_overlap(TE, [t, t, t], ident, ident)[0] == (gap < 0)
+        assert pair_overlap(TE, [-t, -t, -t], ident, ident)[0] == (gap < 0)
+
+
 def test_pair_overlap_closed_forms_ellipsoid():
     """Coaxial spheroids overlap iff |dz| < 2 C; coplanar ones (same axis, separation in the equatorial plane) iff the
     distance is < 2 A; an edge-on spheroid above a flat one (axes perpendicular) iff the gap is < A + C."""
@@ -165,7 +202,7 @@ def test_spherodisk_volume_formula():
     assert abs(workloads.spherodisk_volume(0.4, 0.1) - _gold("spherodisk_volume")) < 1e-6
 
 
-@pytest.mark.parametrize("params", [HB, SD, EL])
+@pytest.mark.parametrize("params", [HB, SD, EL, TE])
 def test_dep_overlap_vs_point_cloud(params):
     """Predicate == (distance from the depletant centre to the solid < r_d), by brute force."""
     rng = np.random.default_rng(11)
@@ -180,13 +217,13 @@ def test_dep_overlap_vs_point_cloud(params):
     got = dep_overlap(params, q, pts_world)
     band = 0.012                                    # cloud resolution
     sure_in, sure_out = dist < rd - band, dist > rd + band
-    assert sure_in.sum() > 300 and sure_out.sum() > 300
+    assert sure_in.sum() > 200 and sure_out.sum() > 300
     assert got[sure_in].all()
     assert not got[sure_out].any()
 
 
 # ----------------------------------------------------------------------------------- support function
-@pytest.mark.parametrize("params", [HB, SD, EL])
+@pytest.mark.parametrize("params", [HB, SD, EL, TE])
 def test_support_is_argmax_over_cloud(olib, params):
     rng = np.random.default_rng(12)
     cloud = shape_cloud(params, 100000, rng)
@@ -212,6 +249,8 @@ def test_support_is_argmax_over_cloud(olib, params):
             exp = {(0, 0, 1): 0.0, (0, 0, -1): 0.5, (1, 0, 0): 0.5}[tuple(n)]
         elif params["shape"] == "ellipsoid":
             exp = {(0, 0, 1): 0.25, (0, 0, -1): 0.25, (1, 0, 0): 0.5}[tuple(n)]
+        elif params["shape"] == "tetrahedron":
+            exp = 0.5 / math.sqrt(3.0)                 # an edge midpoint direction: two vertices tie
         else:
             exp = {(0, 0, 1): 0.1, (0, 0, -1): 0.1, (1, 0, 0): 0.5}[tuple(n)]
         assert abs(float(out @ nv) - exp) < 1e-6
@@ -293,6 +332,10 @@ def _gauge(params):
     if params["shape"] == "halfball":
         R = 0.5 * params["sigma_c"]
         return lambda b: max(np.linalg.norm(b) - R, b[2])
+    if params["shape"] == "tetrahedron":
+        s = 0.5 / math.sqrt(3.0)
+        U = TET_V / s
+        return lambda b: max(-(U @ b) - s) / math.sqrt(3.0)        # signed distance to the nearest face plane
     if params["shape"] == "ellipsoid":
         A, Cc = params["disk_a"], params["disk_s"]
         # convex, <= 0 inside, and at least as large as the signed distance scaled by 1/A near the surface
@@ -324,7 +367,7 @@ def _deepest_common_point(params, rho, qA, qB):
     return best
 
 
-@pytest.mark.parametrize("params", [HB, SD, EL])
+@pytest.mark.parametrize("params", [HB, SD, EL, TE])
 def test_pair_overlap_vs_convex_program(params):
     """Random poses inside the circumsphere range: MPR's verdict == sign of the fp64 convex program,
     outside a contact band."""

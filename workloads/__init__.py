@@ -30,7 +30,7 @@ def spherodisk_volume(a: float, s: float) -> float:
 class Config:
     name: str
     N: int
-    shape: str            # "sphere" | "halfball" | "spherodisk" | "ellipsoid"
+    shape: str            # "sphere" | "halfball" | "spherodisk" | "ellipsoid" | "tetrahedron"
     phi_c: float          # colloid packing fraction
     q: float              # sigma_d / sigma_c
     phi_d_r: tuple        # reservoir packing fraction(s) of the depletants
@@ -38,7 +38,7 @@ class Config:
     a_max: float
     n_trial: int
     sweeps: int
-    init: str             # "rsa" | "fcc" | "sc"
+    init: str             # "rsa" | "fcc" | "sc" | "sca"
     sigma_c: float = 1.0  # circumsphere diameter
     disk_a: float = 0.0
     disk_s: float = 0.0
@@ -50,6 +50,8 @@ class Config:
             return SPHERE_VOL * self.sigma_c ** 3
         if self.shape == "halfball":
             return HALFBALL_VOL * self.sigma_c ** 3
+        if self.shape == "tetrahedron":        # regular, circumradius sigma_c / 2: edge a = R sqrt(8/3), V = a^3 / (6 sqrt 2)
+            return (0.5 * self.sigma_c * math.sqrt(8.0 / 3.0)) ** 3 / (6.0 * math.sqrt(2.0))
         if self.shape == "ellipsoid":          # oblate spheroid, semi-axes (disk_a, disk_a, disk_s)
             return 4.0 * math.pi * self.disk_a ** 2 * self.disk_s / 3.0
         return spherodisk_volume(self.disk_a, self.disk_s)
@@ -84,6 +86,10 @@ _CONFIGS = {
     # a = b = 0.5, c = 0.25, depletant radius 0.25, phi_p^r = 0.40, n_trial >~ 10), here 32^3 of them at phi_c = 0.10
     # (the paper's 500 at phi_c = 0.01 would leave every neighbourhood empty) with C4's step sizes
     "C6": Config("C6", 32768, "ellipsoid", 0.10, 0.50, (0.40,), 0.1, 0.1, 10, 200, "sc", disk_a=0.5, disk_s=0.25),
+    # NEXT-2, second new shape: regular tetrahedra (Fig. 1 L21), circumradius 0.5, all with the same orientation
+    # on a 32^3 lattice of spacing 0.685 (equally oriented tetrahedra are disjoint iff the lattice vector lies outside
+    # their difference body, a cuboctahedron reaching 0.577 along the axes), C4's depletants and step sizes
+    "C7": Config("C7", 32768, "tetrahedron", 0.20, 0.20, (0.25,), 0.1, 0.1, 0, 200, "sca"),
 }
 
 
@@ -177,6 +183,14 @@ def generate(cfg: Config):
             raise ValueError("fcc lattice too dense for this box")
         keep = np.sort(rng.permutation(len(sites))[:N])
         pos = sites[keep]
+    elif cfg.init == "sca":
+        n = int(round(N ** (1.0 / 3.0)))
+        if n ** 3 != N:
+            raise ValueError("simple-cubic initial state needs N = n^3")
+        pos = _sc_sites(n, L)
+        if cfg.shape != "tetrahedron" or L / n < 0.6 * cfg.sigma_c:
+            raise ValueError("aligned lattice: tetrahedra at spacing >= 0.6 circumsphere diameters only")
+        quat = np.tile(np.array([1.0, 0.0, 0.0, 0.0]), (N, 1))
     elif cfg.init == "sc":
         n = int(round(N ** (1.0 / 3.0)))
         if n ** 3 != N:
@@ -184,7 +198,7 @@ def generate(cfg: Config):
         pos = _sc_sites(n, L)
         spacing = L / n
         quat = _random_quats(N, rng)
-        if cfg.shape in ("halfball", "ellipsoid"):
+        if cfg.shape in ("halfball", "ellipsoid", "tetrahedron"):
             if spacing < cfg.sigma_c * 1.0001:
                 raise ValueError("circumspheres of the lattice overlap")
         elif cfg.shape == "spherodisk":
