@@ -36,11 +36,12 @@ import workloads  # noqa: E402
 OPS_PER_NEEDED_DEPLETANT = {"sphere": 131.0,      # 1.91 x 62 + old/new pose tests 11 + ~2 neighbour tests
                             "halfball": 167.0,    # + 15 + 15 closed-form new/old tests + 0.07 n_nbr x 25
                             "spherodisk": 167.0,
-                            "ellipsoid": 420.0}    # + two point-to-ellipse distances of ~125 ops (6 Newton steps) instead of closed forms
+                            "ellipsoid": 420.0,
+                            "tetrahedron": 500.0}  # frame + point-to-tetrahedron distance (one or two faces) for the new and the old pose    # + two point-to-ellipse distances of ~125 ops (6 Newton steps) instead of closed forms
 OPS_PER_MOVE = {"sphere": 500.0,                  # 3 Philox blocks, 27-cell walk (~20 candidates x 12 + 9 rows x 8), table search, commit
                 "halfball": 1500.0,               # + axis staging, ~2 support-function pair tests of ~400 ops (a6)
-                "spherodisk": 1500.0, "ellipsoid": 1500.0}
-OPS_PER_CB_REINSERTION = {"sphere": 150.0, "halfball": 190.0, "spherodisk": 190.0, "ellipsoid": 440.0}   # 1.91 x 62 + both pose tests + neighbour tests
+                "spherodisk": 1500.0, "ellipsoid": 1500.0, "tetrahedron": 2000.0}
+OPS_PER_CB_REINSERTION = {"sphere": 150.0, "halfball": 190.0, "spherodisk": 190.0, "ellipsoid": 440.0, "tetrahedron": 520.0}   # 1.91 x 62 + both pose tests + neighbour tests
 PHILOX_BLOCKS_PER_DEPLETANT = 6.0 / 3.141592653589793
 BYTES_PER_PARTICLE_PER_PASS = 16.0 # every pass reads the cell-ordered float4 array once (re-reads by neighbouring cells are L2 hits)
 BYTES_PER_CELL_PER_PASS = 4.0      # ... and each cell_start word once

@@ -35,8 +35,11 @@ typedef enum {
   HPMC_SPHERE = 0,     /* sphere of diameter sigma_c */
   HPMC_HALFBALL = 1,   /* {x: |x| <= sigma_c/2, x.z_body <= 0}: flat face through the pose centre, outward normal +z_body */
   HPMC_SPHERODISK = 2, /* Minkowski sum of a flat disk (radius disk_a, normal z_body) and a ball (radius disk_s) */
-  HPMC_ELLIPSOID = 3   /* oblate spheroid, semi-axes (disk_a, disk_a, disk_s), disk_a >= disk_s > 0, short axis z_body: the paper's
+  HPMC_TETRAHEDRON = 4, /* regular tetrahedron with circumradius sigma_c / 2, body-frame vertices (sigma_c / (2 sqrt 3)) x
+                          {(1,1,1), (1,-1,-1), (-1,1,-1), (-1,-1,1)} (Fig. 1 L21; NEXT-2, reading R-N2b) */
+  HPMC_ELLIPSOID = 3,  /* oblate spheroid, semi-axes (disk_a, disk_a, disk_s), disk_a >= disk_s > 0, short axis z_body: the paper's
                           discoids (reading R-N2); sigma_c must equal 2 disk_a */
+  HPMC_SHAPE_COUNT = 5
 } hpmc_shape;
 
 typedef enum {

@@ -15,7 +15,7 @@ COUNTER_NAMES = (
     "rej_depletant", "rej_cb", "dep_drawn", "dep_needed", "dep_evaluated", "cb_reinsertions",
     "philox_blocks",
 )
-SHAPES = {"sphere": 0, "halfball": 1, "spherodisk": 2, "ellipsoid": 3}
+SHAPES = {"sphere": 0, "halfball": 1, "spherodisk": 2, "ellipsoid": 3, "tetrahedron": 4}
 OPT_SHELL, OPT_ROSENBLUTH = 1, 2          # hpmc_set_options
 
 EXPORTS = (

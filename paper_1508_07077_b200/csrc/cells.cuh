@@ -139,7 +139,7 @@ __global__ void __launch_bounds__(256) k_fill(const uint32_t* __restrict__ cid, 
   cell_pid[cell_start[cid[i]] + rank[i]] = (uint32_t)i;
 }
 
-template <bool ANISO>
+template <int SHAPE>
 __global__ void __launch_bounds__(256) k_sort_write(const uint32_t* __restrict__ cell_start, int ncell,
                                                     uint32_t* __restrict__ cell_pid, const float4* __restrict__ pos,
                                                     const float4* __restrict__ quat, float4* __restrict__ cpos,
@@ -158,10 +158,7 @@ __global__ void __launch_bounds__(256) k_sort_write(const uint32_t* __restrict__
     float4 p = pos[i];
     p.w = __uint_as_float(i);
     cpos[s] = p;
-    if (ANISO) {
-      const V3 a = quat_axis(as_q(quat[i]));
-      caxis[s] = make_float4(a.x, a.y, a.z, 0.0f);
-    }
+    if (SHAPE != SH_SPHERE) caxis[s] = as_f4(ori_of<SHAPE>(as_q(quat[i])));     // body axis, or the quaternion (tetrahedron)
   }
 }
 

@@ -10,7 +10,7 @@
 
 namespace hpmc {
 
-enum : int { SH_SPHERE = 0, SH_HALFBALL = 1, SH_SPHERODISK = 2, SH_ELLIPSOID = 3 };
+enum : int { SH_SPHERE = 0, SH_HALFBALL = 1, SH_SPHERODISK = 2, SH_ELLIPSOID = 3, SH_TETRAHEDRON = 4 };
 
 struct Geo {              // derived constants, computed once on the host in fp32
   float L, halfL, w;      // box edge, L/2, cell width
@@ -46,6 +46,20 @@ __device__ __forceinline__ V3 quat_axis(Q4 q) {
   return V3{2.0f * (q.x * q.z + q.w * q.y), 2.0f * (q.y * q.z - q.w * q.x), 1.0f - 2.0f * (q.x * q.x + q.y * q.y)};
 }
 
+// Orientation as the shape tests need it: the body z axis (x, y, z; w unused) for the bodies of revolution (R-S19), the
+// whole unit quaternion (x = q.w, y = q.x, z = q.y, w = q.z) for the tetrahedron (R-N2b).  One float4 either way: the
+// cell-ordered orientation array, the shared-memory records and the neighbour pool hold it as it is.
+struct Ori { float x, y, z, w; };
+template <int SHAPE>
+__device__ __forceinline__ Ori ori_of(Q4 q) {
+  if (SHAPE == SH_TETRAHEDRON) return Ori{q.w, q.x, q.y, q.z};
+  const V3 a = quat_axis(q);
+  return Ori{a.x, a.y, a.z, 0.0f};
+}
+__device__ __forceinline__ Ori as_ori(float4 f) { return Ori{f.x, f.y, f.z, f.w}; }
+__device__ __forceinline__ float4 as_f4(Ori o) { return make_float4(o.x, o.y, o.z, o.w); }
+__device__ __forceinline__ V3 axis_of(Ori o) { return V3{o.x, o.y, o.z}; }
+
 // Cayley rotation move (R-S6): q' = normalise((1,v) (x) q), multiplication on the left (space frame)
 __device__ __forceinline__ Q4 rotate_cayley(Q4 q, V3 v) {
   const float pw = q.w - ((v.x * q.x + v.y * q.y) + v.z * q.z);
@@ -55,6 +69,63 @@ __device__ __forceinline__ Q4 rotate_cayley(Q4 q, V3 v) {
   const float n2 = (pw * pw + px * px) + (py * py + pz * pz);
   const float n = __fsqrt_rn(n2);
   return Q4{__fdiv_rn(pw, n), __fdiv_rn(px, n), __fdiv_rn(py, n), __fdiv_rn(pz, n)};
+}
+
+// R-N2b: regular tetrahedron, circumradius Rh = sigma_c / 2, body-frame vertices s u_i with s = Rh 0.57735026f and
+// u_0 = (1,1,1), u_1 = (1,-1,-1), u_2 = (-1,1,-1), u_3 = (-1,-1,1); the face opposite vertex i lies in the plane u_i . x = -s.
+struct Frame { V3 ex, ey, ez; };               // body axes in the space frame: columns of the rotation matrix of q
+__device__ __forceinline__ Frame frame_of(Ori o) {
+  const float w = o.x, x = o.y, y = o.z, z = o.w;
+  Frame f;
+  f.ex = V3{1.0f - 2.0f * (y * y + z * z), 2.0f * (x * y + w * z), 2.0f * (x * z - w * y)};
+  f.ey = V3{2.0f * (x * y - w * z), 1.0f - 2.0f * (x * x + z * z), 2.0f * (y * z + w * x)};
+  f.ez = V3{2.0f * (x * z + w * y), 2.0f * (y * z - w * x), 1.0f - 2.0f * (x * x + y * y)};
+  return f;
+}
+__device__ __forceinline__ V3 tet_u(int i) {
+  return V3{(i & 2) ? -1.0f : 1.0f, (i == 1 || i == 3) ? -1.0f : 1.0f, (i == 1 || i == 2) ? -1.0f : 1.0f};
+}
+// squared distance from p to the triangle (a, b, c): closest-point regions by barycentric signs, only + x /
+__device__ __forceinline__ float tri_dist2(V3 p, V3 a, V3 b, V3 c) {
+  const V3 ab = b - a, ac = c - a, ap = p - a;
+  const float d1 = dot3(ab, ap), d2 = dot3(ac, ap);
+  if (d1 <= 0.0f && d2 <= 0.0f) return dot3(ap, ap);
+  const V3 bp = p - b;
+  const float d3 = dot3(ab, bp), d4 = dot3(ac, bp);
+  if (d3 >= 0.0f && d4 <= d3) return dot3(bp, bp);
+  const float vc = d1 * d4 - d3 * d2;
+  if (vc <= 0.0f && d1 >= 0.0f && d3 <= 0.0f) { const float v = __fdiv_rn(d1, d1 - d3); const V3 e = ap - ab * v; return dot3(e, e); }
+  const V3 cp = p - c;
+  const float d5 = dot3(ab, cp), d6 = dot3(ac, cp);
+  if (d6 >= 0.0f && d5 <= d6) return dot3(cp, cp);
+  const float vb = d5 * d2 - d1 * d6;
+  if (vb <= 0.0f && d2 >= 0.0f && d6 <= 0.0f) { const float w = __fdiv_rn(d2, d2 - d6); const V3 e = ap - ac * w; return dot3(e, e); }
+  const float va = d3 * d6 - d5 * d4;
+  if (va <= 0.0f && (d4 - d3) >= 0.0f && (d5 - d6) >= 0.0f) {
+    const float w = __fdiv_rn(d4 - d3, (d4 - d3) + (d5 - d6));
+    const V3 e = bp - (c - b) * w;
+    return dot3(e, e);
+  }
+  const float den = __fdiv_rn(1.0f, va + vb + vc);
+  const float v = vb * den, w = vc * den;
+  const V3 e = ap - (ab * v + ac * w);
+  return dot3(e, e);
+}
+// depletant centre at body-frame point b vs the tetrahedron: inside, or closer than r_d to a face it lies in front of
+__device__ __forceinline__ bool near_tetrahedron(float s, float rd2, V3 b) {
+  bool inside = true;
+  float best = 3.0e38f;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const V3 u = tet_u(i);
+    const float h = (u.x * b.x + u.y * b.y) + u.z * b.z;
+    if (h < -s) {
+      inside = false;
+      const float d2 = tri_dist2(b, tet_u((i + 1) & 3) * s, tet_u((i + 2) & 3) * s, tet_u((i + 3) & 3) * s);
+      if (d2 < best) best = d2;
+    }
+  }
+  return inside || best < rd2;
 }
 
 // R-N2 (oblate spheroid x^2/A^2 + z^2/C^2 <= 1 in cylindrical body coordinates, the paper's discoids L228): is the point
@@ -83,10 +154,15 @@ __device__ __forceinline__ bool near_spheroid(float A, float Cc, float rd2, floa
 
 // Does a depletant centred at d (relative to the colloid centre) overlap the colloid with body axis a?
 template <int SHAPE>
-__device__ __forceinline__ bool dep_overlap(const Geo& g, V3 d, V3 a) {
+__device__ __forceinline__ bool dep_overlap(const Geo& g, V3 d, Ori o) {
   const float d2 = dot3(d, d);
   if (!(d2 < g.Rins2)) return false;
   if (SHAPE == SH_SPHERE) return true;
+  if (SHAPE == SH_TETRAHEDRON) {
+    const Frame f = frame_of(o);
+    return near_tetrahedron(g.Rh * 0.57735026f, g.rd2, V3{dot3(d, f.ex), dot3(d, f.ey), dot3(d, f.ez)});
+  }
+  const V3 a = axis_of(o);
   const float bz = dot3(d, a);
   if (SHAPE == SH_ELLIPSOID) {
     const V3 p = V3{d.x - bz * a.x, d.y - bz * a.y, d.z - bz * a.z};
@@ -108,7 +184,23 @@ __device__ __forceinline__ bool dep_overlap(const Geo& g, V3 d, V3 a) {
 }
 
 template <int SHAPE>
-__device__ __forceinline__ V3 support(const Geo& g, V3 a, V3 n) {
+__device__ __forceinline__ V3 support(const Geo& g, Ori o, V3 n) {
+  if (SHAPE == SH_TETRAHEDRON) {               // the vertex with the largest projection (first one on ties)
+    const Frame f = frame_of(o);
+    const V3 nb = V3{dot3(n, f.ex), dot3(n, f.ey), dot3(n, f.ez)};
+    int best = 0;
+    float hb = (nb.x + nb.y) + nb.z;
+#pragma unroll
+    for (int i = 1; i < 4; ++i) {
+      const V3 u = tet_u(i);
+      const float h = (u.x * nb.x + u.y * nb.y) + u.z * nb.z;
+      if (h > hb) { hb = h; best = i; }
+    }
+    const float s = g.Rh * 0.57735026f;
+    const V3 u = tet_u(best);
+    return (f.ex * (s * u.x) + f.ey * (s * u.y)) + f.ez * (s * u.z);
+  }
+  const V3 a = axis_of(o);
   const float nz = dot3(n, a);
   if (SHAPE == SH_HALFBALL) {
     if (nz <= 0.0f) {
@@ -139,7 +231,7 @@ __device__ __forceinline__ V3 support(const Geo& g, V3 a, V3 n) {
 }
 
 template <int SHAPE>
-__device__ __forceinline__ V3 support_diff(const Geo& g, V3 rho, V3 aA, V3 aB, V3 n) {
+__device__ __forceinline__ V3 support_diff(const Geo& g, V3 rho, Ori aA, Ori aB, V3 n) {
   const V3 sb = support<SHAPE>(g, aB, n);
   const V3 sa = support<SHAPE>(g, aA, neg(n));
   return (sb + rho) - sa;
@@ -150,11 +242,11 @@ __device__ __forceinline__ V3 support_diff(const Geo& g, V3 rho, V3 aA, V3 aB, V
 
 // Minkowski portal refinement on the full convex shapes: A at the origin (axis aA), B at rho (axis aB).
 template <int SHAPE>
-__device__ __noinline__ bool mpr_overlap(const Geo& g, V3 rho, V3 aA, V3 aB) {
+__device__ __noinline__ bool mpr_overlap(const Geo& g, V3 rho, Ori aA, Ori aB) {
   V3 cA = V3{0.0f, 0.0f, 0.0f}, cB = rho;
   if (SHAPE == SH_HALFBALL) {
-    cA = neg(aA * g.cen);
-    cB = rho - aB * g.cen;
+    cA = neg(axis_of(aA) * g.cen);
+    cB = rho - axis_of(aB) * g.cen;
   }
   V3 v0 = cB - cA;
   if (is_zero(v0)) v0 = V3{1e-5f, 0.0f, 0.0f};
@@ -197,7 +289,7 @@ __device__ __noinline__ bool mpr_overlap(const Geo& g, V3 rho, V3 aA, V3 aB) {
 }
 
 template <int SHAPE>
-__device__ __forceinline__ bool pair_overlap(const Geo& g, V3 rho, V3 aA, V3 aB) {
+__device__ __forceinline__ bool pair_overlap(const Geo& g, V3 rho, Ori aA, Ori aB) {
   const float r2 = dot3(rho, rho);
   if (!(r2 < g.dcirc2)) return false;
   if (SHAPE == SH_SPHERE) return true;

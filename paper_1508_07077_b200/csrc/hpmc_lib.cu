@@ -355,7 +355,7 @@ int hpmc_init(hpmc_ctx** out, const hpmc_params* p, int64_t N, float* d_pos4, fl
   if (N <= 0 || N > 0x7fffffff) return fail(nullptr, HPMC_E_BADARG, "hpmc_init: N out of range");
   if (!(p->box_L > 0.0f) || !(p->sigma_c > 0.0f) || p->sigma_d < 0.0f || p->d_max_cap < 0.0f)
     return fail(nullptr, HPMC_E_BADARG, "hpmc_init: bad geometry parameters");
-  if (p->shape < HPMC_SPHERE || p->shape > HPMC_ELLIPSOID) return fail(nullptr, HPMC_E_BADARG, "hpmc_init: bad shape");
+  if (p->shape < HPMC_SPHERE || p->shape > HPMC_TETRAHEDRON) return fail(nullptr, HPMC_E_BADARG, "hpmc_init: bad shape");
   if (p->shape == HPMC_ELLIPSOID) {
     // oblate spheroid (disk_a, disk_a, disk_s): sigma_c is the circumsphere diameter 2 disk_a
     if (!(p->disk_s > 0.0f) || !(p->disk_a >= p->disk_s) ||
@@ -436,7 +436,8 @@ int hpmc_init(hpmc_ctx** out, const hpmc_params* p, int64_t N, float* d_pos4, fl
       case HPMC_SPHERE: rc = setup_moveq<SH_SPHERE, false>(ctx); if (!rc) rc = setup_moveq<SH_SPHERE, true>(ctx); break;
       case HPMC_HALFBALL: rc = setup_moveq<SH_HALFBALL, false>(ctx); if (!rc) rc = setup_moveq<SH_HALFBALL, true>(ctx); break;
       case HPMC_SPHERODISK: rc = setup_moveq<SH_SPHERODISK, false>(ctx); if (!rc) rc = setup_moveq<SH_SPHERODISK, true>(ctx); break;
-      default: rc = setup_moveq<SH_ELLIPSOID, false>(ctx); if (!rc) rc = setup_moveq<SH_ELLIPSOID, true>(ctx); break;
+      case HPMC_ELLIPSOID: rc = setup_moveq<SH_ELLIPSOID, false>(ctx); if (!rc) rc = setup_moveq<SH_ELLIPSOID, true>(ctx); break;
+      default: rc = setup_moveq<SH_TETRAHEDRON, false>(ctx); if (!rc) rc = setup_moveq<SH_TETRAHEDRON, true>(ctx); break;
     }
     if (rc) { g_init_error = ctx->err; hpmc_destroy(ctx); return rc; }
   }
@@ -493,11 +494,14 @@ int hpmc_build_cells(hpmc_ctx* ctx, uint32_t seed, uint32_t step) {
   k_fill<<<nb, 256, 0, st>>>(ctx->d_cid, ctx->d_rank, ctx->d_cell_start, N, ctx->d_cell_pid);
   const int cbk = (ctx->ncell + 255) / 256;
   if (ctx->p.shape == HPMC_SPHERE)
-    k_sort_write<false><<<cbk, 256, 0, st>>>(ctx->d_cell_start, ctx->ncell, ctx->d_cell_pid, ctx->d_pos, ctx->d_quat,
-                                             ctx->d_cpos, ctx->d_caxis);
-  else
-    k_sort_write<true><<<cbk, 256, 0, st>>>(ctx->d_cell_start, ctx->ncell, ctx->d_cell_pid, ctx->d_pos, ctx->d_quat,
-                                            ctx->d_cpos, ctx->d_caxis);
+    k_sort_write<SH_SPHERE><<<cbk, 256, 0, st>>>(ctx->d_cell_start, ctx->ncell, ctx->d_cell_pid, ctx->d_pos, ctx->d_quat,
+                                                 ctx->d_cpos, ctx->d_caxis);
+  else if (ctx->p.shape == HPMC_TETRAHEDRON)       // cell-ordered orientation = the quaternion itself
+    k_sort_write<SH_TETRAHEDRON><<<cbk, 256, 0, st>>>(ctx->d_cell_start, ctx->ncell, ctx->d_cell_pid, ctx->d_pos, ctx->d_quat,
+                                                      ctx->d_cpos, ctx->d_caxis);
+  else                                             // bodies of revolution: the body z axis
+    k_sort_write<SH_HALFBALL><<<cbk, 256, 0, st>>>(ctx->d_cell_start, ctx->ncell, ctx->d_cell_pid, ctx->d_pos, ctx->d_quat,
+                                                   ctx->d_cpos, ctx->d_caxis);
   CU(cudaGetLastError());
   ctx->built = true; ctx->b_seed = seed; ctx->b_step = step;
   return HPMC_OK;
@@ -518,6 +522,7 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
     float rin = ctx->g.Rins;
     if (ctx->p.shape == HPMC_HALFBALL) rin = ctx->g.rd;
     else if (ctx->p.shape == HPMC_SPHERODISK || ctx->p.shape == HPMC_ELLIPSOID) rin = ctx->g.sdisk + ctx->g.rd;
+    else if (ctx->p.shape == HPMC_TETRAHEDRON) rin = ctx->g.Rh * 0.33333334f + ctx->g.rd;
     sh_Rin = rin - 1.7320508f * d_max;
     if (sh_Rin < 0.0f) sh_Rin = 0.0f;
     const double Ri = (double)sh_Rin;
@@ -577,7 +582,8 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
         case HPMC_SPHERE: rc2 = cb ? launch_moveq<SH_SPHERE, true>(ctx, a, pt, p8) : launch_moveq<SH_SPHERE, false>(ctx, a, pt, p8); break;
         case HPMC_HALFBALL: rc2 = cb ? launch_moveq<SH_HALFBALL, true>(ctx, a, pt, p8) : launch_moveq<SH_HALFBALL, false>(ctx, a, pt, p8); break;
         case HPMC_SPHERODISK: rc2 = cb ? launch_moveq<SH_SPHERODISK, true>(ctx, a, pt, p8) : launch_moveq<SH_SPHERODISK, false>(ctx, a, pt, p8); break;
-        default: rc2 = cb ? launch_moveq<SH_ELLIPSOID, true>(ctx, a, pt, p8) : launch_moveq<SH_ELLIPSOID, false>(ctx, a, pt, p8); break;
+        case HPMC_ELLIPSOID: rc2 = cb ? launch_moveq<SH_ELLIPSOID, true>(ctx, a, pt, p8) : launch_moveq<SH_ELLIPSOID, false>(ctx, a, pt, p8); break;
+        default: rc2 = cb ? launch_moveq<SH_TETRAHEDRON, true>(ctx, a, pt, p8) : launch_moveq<SH_TETRAHEDRON, false>(ctx, a, pt, p8); break;
       }
       if (rc2) return rc2;
     }
@@ -590,7 +596,8 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
         case HPMC_SPHERE: launch_move<SH_SPHERE>(ctx, a, cb); break;
         case HPMC_HALFBALL: launch_move<SH_HALFBALL>(ctx, a, cb); break;
         case HPMC_SPHERODISK: launch_move<SH_SPHERODISK>(ctx, a, cb); break;
-        default: launch_move<SH_ELLIPSOID>(ctx, a, cb); break;
+        case HPMC_ELLIPSOID: launch_move<SH_ELLIPSOID>(ctx, a, cb); break;
+        default: launch_move<SH_TETRAHEDRON>(ctx, a, cb); break;
       }
     }
   }
@@ -618,7 +625,8 @@ int hpmc_free_volume(hpmc_ctx* ctx, uint32_t seed, uint32_t step, int64_t n_samp
       case HPMC_SPHERE: k_free_volume<SH_SPHERE><<<grid, 256, 0, ctx->stream>>>(ctx->g, key, ctx->shift[0], ctx->shift[1], ctx->shift[2], n_samples, ctx->d_cpos, ctx->d_caxis, ctx->d_cell_start, d_cnt); break;
       case HPMC_HALFBALL: k_free_volume<SH_HALFBALL><<<grid, 256, 0, ctx->stream>>>(ctx->g, key, ctx->shift[0], ctx->shift[1], ctx->shift[2], n_samples, ctx->d_cpos, ctx->d_caxis, ctx->d_cell_start, d_cnt); break;
       case HPMC_SPHERODISK: k_free_volume<SH_SPHERODISK><<<grid, 256, 0, ctx->stream>>>(ctx->g, key, ctx->shift[0], ctx->shift[1], ctx->shift[2], n_samples, ctx->d_cpos, ctx->d_caxis, ctx->d_cell_start, d_cnt); break;
-      default: k_free_volume<SH_ELLIPSOID><<<grid, 256, 0, ctx->stream>>>(ctx->g, key, ctx->shift[0], ctx->shift[1], ctx->shift[2], n_samples, ctx->d_cpos, ctx->d_caxis, ctx->d_cell_start, d_cnt); break;
+      case HPMC_ELLIPSOID: k_free_volume<SH_ELLIPSOID><<<grid, 256, 0, ctx->stream>>>(ctx->g, key, ctx->shift[0], ctx->shift[1], ctx->shift[2], n_samples, ctx->d_cpos, ctx->d_caxis, ctx->d_cell_start, d_cnt); break;
+      default: k_free_volume<SH_TETRAHEDRON><<<grid, 256, 0, ctx->stream>>>(ctx->g, key, ctx->shift[0], ctx->shift[1], ctx->shift[2], n_samples, ctx->d_cpos, ctx->d_caxis, ctx->d_cell_start, d_cnt); break;
     }
     ctx->launches += 1;
   }

@@ -98,7 +98,8 @@ __device__ __forceinline__ V3 dep_position(const MoveArgs& A, uint32_t pid, uint
 
 template <int SHAPE>
 struct MoveCtx {       // per-move state shared by the depletant predicates
-  V3 rho_old, a_old, a_new;
+  V3 rho_old;
+  Ori a_old, a_new;
   const float4* nb;    // shared memory: neighbour centres relative to the new centre
   const float4* ax;    // shared memory: neighbour axes
   int nnb;
@@ -108,8 +109,8 @@ template <int SHAPE>
 __device__ __forceinline__ bool free_of_nbrs(const Geo& g, const MoveCtx<SHAPE>& m, V3 d) {
   for (int j = 0; j < m.nnb; ++j) {
     const float4 r = m.nb[j];
-    V3 a = V3{0.0f, 0.0f, 1.0f};
-    if (SHAPE != SH_SPHERE) { const float4 t = m.ax[j]; a = V3{t.x, t.y, t.z}; }
+    Ori a = Ori{0.0f, 0.0f, 1.0f, 0.0f};
+    if (SHAPE != SH_SPHERE) a = as_ori(m.ax[j]);
     if (dep_overlap<SHAPE>(g, d - V3{r.x, r.y, r.z}, a)) return false;
   }
   return true;
@@ -152,8 +153,8 @@ __global__ void __launch_bounds__(256) k_free_volume(Geo g, Key10 key, float sx,
         const uint32_t e = part == 0 ? cell_start[rb + x0 + n0] : cell_start[rb + n1];
         for (uint32_t t = b; t < e; ++t) {
           const float4 c = cpos[t];
-          V3 a = V3{0.0f, 0.0f, 1.0f};
-          if (SHAPE != SH_SPHERE) { const float4 ax = caxis[t]; a = V3{ax.x, ax.y, ax.z}; }
+          Ori a = Ori{0.0f, 0.0f, 1.0f, 0.0f};
+          if (SHAPE != SH_SPHERE) a = as_ori(caxis[t]);
           const V3 d = V3{minimg1(g, p.x - c.x), minimg1(g, p.y - c.y), minimg1(g, p.z - c.z)};
           if (dep_overlap<SHAPE>(g, d, a)) { is_free = false; break; }
         }
@@ -283,8 +284,8 @@ __global__ void __launch_bounds__(MOVE_WARPS * 32) k_move(const MoveArgs A) {
 
       MoveCtx<SHAPE> m;
       m.rho_old = V3{minimg1(g, r0.x - r1.x), minimg1(g, r0.y - r1.y), minimg1(g, r0.z - r1.z)};
-      m.a_old = quat_axis(q0);
-      m.a_new = quat_axis(q1);
+      m.a_old = ori_of<SHAPE>(q0);
+      m.a_new = ori_of<SHAPE>(q1);
       m.nb = s_nb[wid];
       m.ax = s_ax[wid];
       m.nnb = nnb;
@@ -293,8 +294,8 @@ __global__ void __launch_bounds__(MOVE_WARPS * 32) k_move(const MoveArgs A) {
       bool hard = false;
       for (int j = lane; j < nnb; j += 32) {
         const float4 r = s_nb[wid][j];
-        V3 aB = V3{0.0f, 0.0f, 1.0f};
-        if (SHAPE != SH_SPHERE) { const float4 t = s_ax[wid][j]; aB = V3{t.x, t.y, t.z}; }
+        Ori aB = Ori{0.0f, 0.0f, 1.0f, 0.0f};
+        if (SHAPE != SH_SPHERE) aB = as_ori(s_ax[wid][j]);
         if (pair_overlap<SHAPE>(g, V3{r.x, r.y, r.z}, m.a_new, aB)) hard = true;
       }
       if (__any_sync(FULL, hard)) out = OUT_HARD;
@@ -398,8 +399,7 @@ __global__ void __launch_bounds__(MOVE_WARPS * 32) k_move(const MoveArgs A) {
         A.cpos[slot] = make_float4(r1.x, r1.y, r1.z, p0.w);
         if (SHAPE != SH_SPHERE && rot) {
           A.quat[pid] = as_f4(q1);
-          const V3 an = quat_axis(q1);
-          A.caxis[slot] = make_float4(an.x, an.y, an.z, 0.0f);
+          A.caxis[slot] = as_f4(ori_of<SHAPE>(q1));
         }
       }
       ++cnt[rot ? C_TRIALS_ROT : C_TRIALS_TRANS];

@@ -136,7 +136,7 @@ struct QSmem {
 };
 
 template <int SHAPE>
-__device__ __forceinline__ bool q_new_only(const Geo& g, V3 d, V3 rho_old, V3 a_old, V3 a_new) {
+__device__ __forceinline__ bool q_new_only(const Geo& g, V3 d, V3 rho_old, Ori a_old, Ori a_new) {
   return dep_overlap<SHAPE>(g, d, a_new) && !dep_overlap<SHAPE>(g, d - rho_old, a_old);
 }
 
@@ -145,8 +145,8 @@ __device__ __forceinline__ bool q_free_of_nbrs(const Geo& g, const float4* pool,
   constexpr int E = QLayout<SHAPE>::ENTRY;
   for (int e = head; e >= 0;) {
     const float4 r = pool[e * E];
-    V3 a = V3{0.0f, 0.0f, 1.0f};
-    if (SHAPE != SH_SPHERE) { const float4 t = pool[e * E + 1]; a = V3{t.x, t.y, t.z}; }
+    Ori a = Ori{0.0f, 0.0f, 1.0f, 0.0f};
+    if (SHAPE != SH_SPHERE) a = as_ori(pool[e * E + 1]);
     if (dep_overlap<SHAPE>(g, d - V3{r.x, r.y, r.z}, a)) return false;
     e = __float_as_int(r.w);
   }
@@ -201,11 +201,8 @@ __device__ __forceinline__ void q_depletant_queue(const QTables& tb, int nalive,
   int c_head = tb.head[m];
   float4 c_rho = tb.rho[m];
   uint32_t c_pid = __float_as_uint(c_rho.w);
-  V3 c_aold = V3{0.f, 0.f, 1.f}, c_anew = V3{0.f, 0.f, 1.f};
-  if (ANISO) {
-    const float4 ao = tb.aold[m], an = tb.anew[m];
-    c_aold = V3{ao.x, ao.y, ao.z}; c_anew = V3{an.x, an.y, an.z};
-  }
+  Ori c_aold = Ori{0.f, 0.f, 1.f, 0.f}, c_anew = Ori{0.f, 0.f, 1.f, 0.f};
+  if (ANISO) { c_aold = as_ori(tb.aold[m]); c_anew = as_ori(tb.anew[m]); }
   volatile uint32_t* v_rejmin = tb.rejmin;
   volatile uint32_t* v_todo = tb.todo;
   uint32_t k = 0, c3 = c3dep, trip = 0;
@@ -239,10 +236,7 @@ __device__ __forceinline__ void q_depletant_queue(const QTables& tb, int nalive,
         j = found;
         m = tb.alive[j];
         c_head = tb.head[m]; c_rho = tb.rho[m]; c_pid = __float_as_uint(c_rho.w);
-        if (ANISO) {
-          const float4 ao = tb.aold[m], an = tb.anew[m];
-          c_aold = V3{ao.x, ao.y, ao.z}; c_anew = V3{an.x, an.y, an.z};
-        }
+        if (ANISO) { c_aold = as_ori(tb.aold[m]); c_anew = as_ori(tb.anew[m]); }
       }
     }
     // the vote is also the reconvergence point: the Philox block below runs with the whole warp together
@@ -463,9 +457,8 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
             s_state[e] = OUT_NONE;
             if (ANISO) {
               s_q1[e] = as_f4(q1);
-              const V3 ao = quat_axis(q0), an = quat_axis(q1);
-              s_aold[e] = make_float4(ao.x, ao.y, ao.z, 0.0f);
-              s_anew[e] = make_float4(an.x, an.y, an.z, 0.0f);
+              s_aold[e] = as_f4(ori_of<SHAPE>(q0));
+              s_anew[e] = as_f4(ori_of<SHAPE>(q1));
             }
           }
         }
@@ -565,8 +558,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
               const uint32_t hi = atomicAdd(&s_scal[3], 1u);
               if (hi < (uint32_t)HCAP) s_hitems[hi] = ((uint32_t)e << 16) | (uint32_t)pe;
               else {
-                const float4 an = s_anew[e];
-                if (mpr_overlap<SHAPE>(g, rho, V3{an.x, an.y, an.z}, V3{axj.x, axj.y, axj.z})) s_state[e] = OUT_HARD;
+                if (mpr_overlap<SHAPE>(g, rho, as_ori(s_anew[e]), as_ori(axj))) s_state[e] = OUT_HARD;
               }
             }
           }
@@ -585,7 +577,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
         const uint32_t itm = s_hitems[i];
         const uint32_t sl = itm >> 16, pe = itm & 0xffffu;
         const float4 r = s_pool[pe * E], ax = s_pool[pe * E + 1], an = s_anew[sl];
-        if (mpr_overlap<SHAPE>(g, V3{r.x, r.y, r.z}, V3{an.x, an.y, an.z}, V3{ax.x, ax.y, ax.z}))
+        if (mpr_overlap<SHAPE>(g, V3{r.x, r.y, r.z}, as_ori(an), as_ori(ax)))
           s_state[sl] = OUT_HARD;
       }
     }
@@ -688,8 +680,8 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
         if (rosen && e2 == ne - 1u) continue;
         const float4 r1f = s_r1[m], rof = s_rho[m];
         const V3 ro = V3{rof.x, rof.y, rof.z};
-        V3 ao = V3{0.f, 0.f, 1.f}, an = V3{0.f, 0.f, 1.f};
-        if (ANISO) { const float4 a0 = s_aold[m], a1 = s_anew[m]; ao = V3{a0.x, a0.y, a0.z}; an = V3{a1.x, a1.y, a1.z}; }
+        Ori ao = Ori{0.f, 0.f, 1.f, 0.f}, an = Ori{0.f, 0.f, 1.f, 0.f};
+        if (ANISO) { ao = as_ori(s_aold[m]); an = as_ori(s_anew[m]); }
         V3 sp = ball_sample(A.key, __float_as_uint(rof.w), kk, tt + (dir << 16), c3cb, g.Rins, g.Rins2, n_blocks);
         bool valid;
         if (dir == 0) {                  // forward: about the old centre, must overlap the old pose only (R-G2)
@@ -771,8 +763,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
         A.cpos[slot] = make_float4(r1f.x, r1f.y, r1f.z, __uint_as_float(pid));
         if (ANISO && rot) {
           A.quat[pid] = s_q1[e];
-          const float4 an = s_anew[e];
-          A.caxis[slot] = make_float4(an.x, an.y, an.z, 0.0f);
+          A.caxis[slot] = s_anew[e];
         }
         atomicAdd(&s_cnt[rot ? C_ACCEPT_ROT : C_ACCEPT_TRANS], 1u);
       } else atomicAdd(&s_cnt[out == OUT_HARD ? C_REJ_HARD : (out == OUT_CB ? C_REJ_CB : C_REJ_DEPLETANT)], 1u);

@@ -224,6 +224,27 @@ def test_c6_oblate_ellipsoids(monkeypatch, n_trial, kernel, options, N, sweeps):
         h.close()
 
 
+@pytest.mark.parametrize("n_trial,kernel,options,N,sweeps", [(0, None, 0, None, 200), (4, "warp", 0, 4096, 60), (20, None, 2, 4096, 40),
+                                                             (0, None, 1, 4096, 60)])
+def test_c7_tetrahedra(monkeypatch, n_trial, kernel, options, N, sweeps):
+    """regular tetrahedra (Fig. 1), the one shape that is not a body of revolution (the
+    kernels stage the whole quaternion per neighbour): plain rule at 32,768 particles on the dense aligned lattice
+    (phi_c = 0.20: many support-function pair tests), CB on both kernels, Rosenbluth weight, shell; free-volume count."""
+    import dataclasses
+    if kernel:
+        monkeypatch.setenv("HPMC_CB_KERNEL", kernel)
+    cfg = dataclasses.replace(workloads.config("C7", N), n_trial=n_trial)
+    pos, quat = workloads.generate(cfg)
+    c = run_parity(cfg, pos, quat, sweeps if FULL else 10, cfg.n_R(), options=options)
+    assert c["accept_rot"] > 0 and c["accept_trans"] > 0 and c["rej_hard"] > 0
+    assert (c["rej_cb"] if n_trial else c["rej_depletant"]) > 0
+    if n_trial == 0 and not options:
+        o, h, dpos, dquat = _mk(cfg, pos, quat)
+        o.build_cells(cfg.seed, 0); h.build_cells(cfg.seed, 0)
+        assert h.free_volume(cfg.seed, 0, 200000) == o.free_volume(cfg.seed, 0, 200000)
+        h.close()
+
+
 def test_one_launch_per_pass_mode(monkeypatch):
     """HPMC_SWEEP_LAUNCHES=8: the item-queue kernel launched once per checkerboard pass (no neighbour waits) instead of
     once per sweep; same bits."""
