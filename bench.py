@@ -314,11 +314,12 @@ def timed_run(hp, torch, cfg, seed, pos, quat, n_R, steps, warmup, flush, step0=
 
 def per_config_lines(hp, torch, alu, pk, flush, clocks):
     """moves/s, depletant insertions/s, us per pass and roofline fraction of the other BASELINE.json configurations
-    (C1, C2 at its four reservoir densities after melting 1000 sweeps at n_R = 0 through the library, C4, C5), each a
-    short device-timed run from its seeded initial state.  Context for the C3 headline, same kernels, same clocks."""
+    (C1, C2 at its four reservoir densities after melting 1000 sweeps at n_R = 0 through the library, C4, C5), of the two
+    NEXT-2 shapes (C6 ellipsoids with n_trial = 10, C7 tetrahedra) and of C3 with the shell option, each a short
+    device-timed run from its seeded initial state.  Context for the C3 headline, same kernels, same clocks."""
     import numpy as np
     out = {}
-    plan = [("C1", 200, 0), ("C2", 50, 0), ("C4", 50, 0), ("C5", 50, 0), ("C3", 10, hp.OPT_SHELL)]
+    plan = [("C1", 200, 0), ("C2", 50, 0), ("C4", 50, 0), ("C5", 50, 0), ("C6", 50, 0), ("C7", 50, 0), ("C3", 10, hp.OPT_SHELL)]
     for name, steps, options in plan:
         cfg = workloads.config(name)
         pos, quat = workloads.generate(cfg)

@@ -105,7 +105,8 @@ void hpmc_destroy(hpmc_ctx* ctx);
  * cell-ordered pose copy.  Call once before every hpmc_sweep with the same (seed, step).  Asynchronous. */
 int hpmc_build_cells(hpmc_ctx* ctx, uint32_t seed, uint32_t step);
 
-/* One sweep = the 8 checkerboard sub-lattice passes in a Philox-permuted order (L180), steps a3-a10.  In every
+/* One sweep = the 8 checkerboard sub-lattice passes in a Philox-permuted order (L180), steps a3-a10, normally ONE
+ * cooperative kernel launch in which a CTA waits between passes only for the CTAs owning neighbouring cells.  In every
  * non-empty active cell one colloid gets a trial move: translation uniform in [-d_max, d_max]^3, or (if
  * a_max > 0, with probability 1/2) a Cayley rotation with parameter vector uniform in the ball of radius a_max.
  *   n_R      depletant reservoir number density (fugacity z_p, L214); 0 = plain hard-particle MC
@@ -171,10 +172,10 @@ int hpmc_step_host(hpmc_ctx* ctx, float* host_pos4, float* host_quat4, uint8_t* 
 /* Number of kernel launches the library has enqueued since init (for bench.py's gpu_launches). */
 int64_t hpmc_launch_count(hpmc_ctx* ctx);
 
-/* Event timing of the move kernel (the dominant kernel): while enabled, the 8 move-kernel launches of every sweep
- * are bracketed by ONE pair of CUDA events on the context's stream (the gaps between the 8 launches are inside the
- * bracket); hpmc_move_kernel_ms synchronises and returns the accumulated milliseconds and the number of launches
- * (8 per sweep) since enabling. */
+/* Event timing of the move kernel (the dominant kernel): while enabled, the move-kernel launch(es) of every sweep -- one
+ * cooperative launch for the 8 passes, or 8 launches (HPMC_SWEEP_LAUNCHES=8, the warp-per-cell kernel) -- are bracketed
+ * by ONE pair of CUDA events on the context's stream (gaps between launches are inside the bracket);
+ * hpmc_move_kernel_ms synchronises and returns the accumulated milliseconds and the number of launches since enabling. */
 int hpmc_time_move_kernel(hpmc_ctx* ctx, int32_t enable);
 int hpmc_move_kernel_ms(hpmc_ctx* ctx, double* ms_total, int64_t* launches);
 

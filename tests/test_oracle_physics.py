@@ -427,7 +427,7 @@ def test_cb_zero_trials_equals_plain_and_zero_density_is_hard_mc():
 
 # ------------------------------------------------------------------ check 1 + structural invariants
 @pytest.mark.parametrize("name,N,sweeps", [("C1", None, 100), ("C2", 2048, 30), ("C3", 4096, 10), ("C4", 512, 40),
-                                            ("C5", 512, 40), ("C6", 512, 40), ("C7", 512, 40)])
+                                            ("C5", 512, 40), ("C6", 512, 40), ("C7", 4096, 15)])
 def test_zero_overlaps_and_bookkeeping(name, N, sweeps):
     cfg = workloads.config(name, N)
     pos, quat = workloads.generate(cfg)
