@@ -447,10 +447,12 @@ def main():
         barrier()
         ce = hh.counters()
         te, (we,) = reduce_over_ranks(e0.elapsed_time(e1), [ce["trials_trans"] + ce["trials_rot"]], "cuda", world)
-        nq = 2 if quat is not None else 1
-        e2e = {"value": we / (te * 1e-3), "unit": "moves/s",
-               "h2d_bytes_per_step": 16 * cfg.N * nq, "d2h_bytes_per_step": 16 * cfg.N * nq + cfg.N,
-               "ms_per_step": te / args.steps}
+        # bytes the library really moved in the last step: whole pose arrays up; outcome codes and, when few particles
+        # moved, only the accepted particles' poses down (hpmc_step_host's sparse download), else the whole arrays
+        h2d, d2h = hh.step_host_bytes()
+        e2e = {"value": we / (te * 1e-3), "unit": "moves/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "ms_per_step": te / args.steps,
+               "note": "d2h = outcome codes (N bytes) + list and poses of the accepted particles (sparse download)"}
         hh.close()
 
     if rank == 0:

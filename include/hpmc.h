@@ -163,11 +163,16 @@ int hpmc_cells(hpmc_ctx* ctx, uint32_t* d_cell_start, uint32_t* d_cell_pid, floa
  * hpmc_upload: host -> device copy of N x float4 centres (and orientations unless NULL).
  * hpmc_download: device -> host copy of centres, orientations and outcome codes (any may be NULL).
  * hpmc_step_host: upload, hpmc_build_cells, hpmc_sweep, download, then synchronise: one whole step with the
- * host<->device traffic inside it. */
+ * host<->device traffic inside it.  The download is sparse when it pays: the move kernel lists the particles it accepted,
+ * the outcome codes (N bytes) and the list length come back first, and if at most N/4 particles moved only their poses
+ * are copied (packed by a gather kernel) and patched into host_pos4 / host_quat4 -- which still hold the uploaded poses
+ * of everybody else -- otherwise the whole arrays.  The host arrays end up exactly as after a full download.
+ * hpmc_step_host_bytes: bytes the last hpmc_step_host moved in each direction. */
 int hpmc_upload(hpmc_ctx* ctx, const float* host_pos4, const float* host_quat4);
 int hpmc_download(hpmc_ctx* ctx, float* host_pos4, float* host_quat4, uint8_t* host_outcome);
 int hpmc_step_host(hpmc_ctx* ctx, float* host_pos4, float* host_quat4, uint8_t* host_outcome, uint32_t seed,
                    uint32_t step, double n_R, float d_max, float a_max, int32_t n_trial);
+int hpmc_step_host_bytes(hpmc_ctx* ctx, int64_t* h2d_bytes, int64_t* d2h_bytes);
 
 /* Number of kernel launches the library has enqueued since init (for bench.py's gpu_launches). */
 int64_t hpmc_launch_count(hpmc_ctx* ctx);

@@ -22,7 +22,7 @@ EXPORTS = (
     "hpmc_init", "hpmc_destroy", "hpmc_build_cells", "hpmc_sweep", "hpmc_run", "hpmc_counters",
     "hpmc_reset_counters", "hpmc_outcomes", "hpmc_grid", "hpmc_cells", "hpmc_upload", "hpmc_download",
     "hpmc_step_host", "hpmc_launch_count", "hpmc_time_move_kernel", "hpmc_move_kernel_ms", "hpmc_last_error",
-    "hpmc_alu_peaks", "hpmc_set_options", "hpmc_free_volume",
+    "hpmc_alu_peaks", "hpmc_set_options", "hpmc_free_volume", "hpmc_step_host_bytes",
 )
 
 
@@ -77,6 +77,7 @@ def load_library() -> C.CDLL:
         "hpmc_sweep": (i32, [vp, u32, u32, f64, f32, f32, i32]),
         "hpmc_run": (i32, [vp, u32, u32, i64, f64, f32, f32, i32]),
         "hpmc_set_options": (i32, [vp, u32]),
+        "hpmc_step_host_bytes": (i32, [vp, P(i64), P(i64)]),
         "hpmc_free_volume": (i32, [vp, u32, u32, i64, P(C.c_uint64)]),
         "hpmc_counters": (i32, [vp, P(Counters)]),
         "hpmc_reset_counters": (i32, [vp]),
@@ -176,6 +177,11 @@ class HPMC:
         out = C.c_uint64(0)
         self._ck(self.L.hpmc_free_volume(self.h, seed, step, int(n_samples), C.byref(out)))
         return int(out.value)
+
+    def step_host_bytes(self):
+        a, b = C.c_int64(0), C.c_int64(0)
+        self._ck(self.L.hpmc_step_host_bytes(self.h, C.byref(a), C.byref(b)))
+        return int(a.value), int(b.value)
 
     def set_options(self, options):
         self._ck(self.L.hpmc_set_options(self.h, int(options)))

@@ -78,6 +78,13 @@ struct hpmc_ctx {
   int move_ctas = 0;
   QPlan plan[2];                       // launch plans of the item-queue move kernel: [0] plain rule, [1] configurational bias
   uint32_t options = 0;                // hpmc_set_options
+  // host-buffer path: accepted-particle list of the sweep in flight, packed poses, pinned staging (hpmc_step_host)
+  uint32_t *d_acc_count = nullptr, *d_acc_list = nullptr, *h_acc_list = nullptr;
+  float4 *d_acc_pack = nullptr, *h_acc_pack = nullptr;
+  uint32_t* h_acc_count = nullptr;
+  bool track_accepts = false;          // set by hpmc_step_host for the sweep it issues
+  size_t acc_cap = 0;                  // entries the sparse download may carry (beyond: full copy)
+  int64_t last_h2d = 0, last_d2h = 0;  // bytes of the last hpmc_step_host
   bool use_queue = true;               // HPMC_MOVE_KERNEL=warp selects the first (warp-per-cell) design
   int cb_kernel = 0;                   // configurational bias: 0 = choose per sweep (n_trial, N), 1 = warp-per-cell kernel, 2 = item-queue kernel (HPMC_CB_KERNEL=warp|queue)
   int64_t launches = 0;
@@ -464,6 +471,10 @@ void hpmc_destroy(hpmc_ctx* ctx) {
   cudaFree(ctx->d_cpos); cudaFree(ctx->d_caxis); cudaFree(ctx->d_cid); cudaFree(ctx->d_rank);
   cudaFree(ctx->d_cell_pid); cudaFree(ctx->d_counts); cudaFree(ctx->d_cell_start); cudaFree(ctx->d_tile_sums);
   cudaFree(ctx->d_outcome); cudaFree(ctx->d_counters); cudaFree(ctx->d_err);
+  cudaFree(ctx->d_acc_count); cudaFree(ctx->d_acc_list); cudaFree(ctx->d_acc_pack);
+  if (ctx->h_acc_list) cudaFreeHost(ctx->h_acc_list);
+  if (ctx->h_acc_pack) cudaFreeHost(ctx->h_acc_pack);
+  if (ctx->h_acc_count) cudaFreeHost(ctx->h_acc_count);
   for (auto& pl : ctx->plan) { cudaFree(pl.d_cta_first); cudaFree(pl.d_done); }
   for (auto& t : ctx->tables) { cudaFree(t.d_T); cudaFree(t.d_G); }
   for (auto& e : ctx->ev) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
@@ -553,6 +564,8 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
   a.ptable = pt->d_T; a.pt_n = pt->n; a.pt_klo = pt->k_lo;
   a.outcome = ctx->d_outcome; a.counters = ctx->d_counters; a.err_flag = ctx->d_err;
   a.options = ctx->options;
+  a.acc_count = ctx->track_accepts ? ctx->d_acc_count : nullptr;
+  a.acc_list = ctx->track_accepts ? ctx->d_acc_list : nullptr;
   a.sh_Rin3 = (sh_Rin * sh_Rin) * sh_Rin;
   a.sh_dR3 = (ctx->g.Rins * ctx->g.Rins) * ctx->g.Rins - a.sh_Rin3;
   const bool cb = n_trial > 0;
@@ -729,15 +742,69 @@ int hpmc_download(hpmc_ctx* ctx, float* host_pos4, float* host_quat4, uint8_t* h
 
 int hpmc_step_host(hpmc_ctx* ctx, float* host_pos4, float* host_quat4, uint8_t* host_outcome, uint32_t seed,
                    uint32_t step, double n_R, float d_max, float a_max, int32_t n_trial) {
+  if (!ctx || !host_pos4) return HPMC_E_BADARG;
+  const int64_t N = ctx->N;
+  const bool has_q = host_quat4 && ctx->d_quat;
+  const size_t per = sizeof(float4) * (has_q ? 2 : 1);
+  if (!ctx->d_acc_list) {
+    // sparse download: the device keeps the list of the particles accepted in the sweep; if it is short, only their
+    // poses come back and are patched into the host arrays (which hold the uploaded poses of all the others)
+    ctx->acc_cap = (size_t)std::max<int64_t>(1, N / 4);
+    CU(cudaMalloc(&ctx->d_acc_count, sizeof(uint32_t)));
+    CU(cudaMalloc(&ctx->d_acc_list, sizeof(uint32_t) * (size_t)N));
+    CU(cudaMalloc(&ctx->d_acc_pack, sizeof(float4) * 2 * ctx->acc_cap));
+    CU(cudaMallocHost(&ctx->h_acc_list, sizeof(uint32_t) * ctx->acc_cap));
+    CU(cudaMallocHost(&ctx->h_acc_pack, sizeof(float4) * 2 * ctx->acc_cap));
+    CU(cudaMallocHost(&ctx->h_acc_count, sizeof(uint32_t)));
+  }
   int rc = hpmc_upload(ctx, host_pos4, host_quat4);
   if (rc) return rc;
+  CU(cudaMemsetAsync(ctx->d_acc_count, 0, sizeof(uint32_t), ctx->stream));
   rc = hpmc_build_cells(ctx, seed, step);
   if (rc) return rc;
+  ctx->track_accepts = true;
   rc = hpmc_sweep(ctx, seed, step, n_R, d_max, a_max, n_trial);
+  ctx->track_accepts = false;
   if (rc) return rc;
-  rc = hpmc_download(ctx, host_pos4, host_quat4, host_outcome);
-  if (rc) return rc;
+  ctx->last_h2d = (int64_t)(sizeof(float4) * N * (has_q ? 2 : 1));
+  ctx->last_d2h = 0;
+  if (host_outcome) {
+    CU(cudaMemcpyAsync(host_outcome, ctx->d_outcome, (size_t)N, cudaMemcpyDeviceToHost, ctx->stream));
+    ctx->last_d2h += N;
+  }
+  CU(cudaMemcpyAsync(ctx->h_acc_count, ctx->d_acc_count, sizeof(uint32_t), cudaMemcpyDeviceToHost, ctx->stream));
+  CU(cudaStreamSynchronize(ctx->stream));
+  const uint32_t n = *ctx->h_acc_count;
+  ctx->last_d2h += 4;
+  if ((size_t)n <= ctx->acc_cap) {
+    if (n > 0) {
+      k_gather_accepted<<<(n + 255) / 256, 256, 0, ctx->stream>>>(ctx->d_acc_list, n, ctx->d_pos, has_q ? ctx->d_quat : nullptr,
+                                                                  ctx->d_acc_pack);
+      ctx->launches += 1;
+      CU(cudaMemcpyAsync(ctx->h_acc_list, ctx->d_acc_list, sizeof(uint32_t) * n, cudaMemcpyDeviceToHost, ctx->stream));
+      CU(cudaMemcpyAsync(ctx->h_acc_pack, ctx->d_acc_pack, per * n, cudaMemcpyDeviceToHost, ctx->stream));
+      CU(cudaStreamSynchronize(ctx->stream));
+      float4* hp4 = reinterpret_cast<float4*>(host_pos4);
+      float4* hq4 = reinterpret_cast<float4*>(host_quat4);
+      for (uint32_t i = 0; i < n; ++i) {
+        const uint32_t pid = ctx->h_acc_list[i];
+        hp4[pid] = ctx->h_acc_pack[i];
+        if (has_q) hq4[pid] = ctx->h_acc_pack[(size_t)n + i];
+      }
+      ctx->last_d2h += (int64_t)((sizeof(uint32_t) + per) * n);
+    }
+  } else {
+    rc = hpmc_download(ctx, host_pos4, host_quat4, nullptr);
+    if (rc) return rc;
+    ctx->last_d2h += (int64_t)(per * N);
+  }
   return check_err_flag(ctx);
+}
+
+int hpmc_step_host_bytes(hpmc_ctx* ctx, int64_t* h2d_bytes, int64_t* d2h_bytes) {
+  if (!ctx || !h2d_bytes || !d2h_bytes) return HPMC_E_BADARG;
+  *h2d_bytes = ctx->last_h2d; *d2h_bytes = ctx->last_d2h;
+  return HPMC_OK;
 }
 
 int64_t hpmc_launch_count(hpmc_ctx* ctx) { return ctx ? ctx->launches : 0; }

@@ -46,6 +46,8 @@ struct MoveArgs {
   uint8_t* outcome;
   unsigned long long* counters;
   int* err_flag;
+  uint32_t* acc_count;                 // host-buffer path: list of the particles accepted this sweep (nullptr: not kept)
+  uint32_t* acc_list;
   uint32_t options;                    // OPT_SHELL | OPT_ROSENBLUTH (hpmc_set_options)
   float sh_Rin3, sh_dR3;               // shell option (R-N1): R_in^3 and R^3 - R_in^3
 };
@@ -164,6 +166,16 @@ __global__ void __launch_bounds__(256) k_free_volume(Geo g, Key10 key, float sx,
   }
   for (int o = 16; o >= 1; o >>= 1) mine += __shfl_xor_sync(0xffffffffu, mine, o);
   if ((threadIdx.x & 31) == 0 && mine) atomicAdd(count, mine);
+}
+
+// Host-buffer path (hpmc_step_host): the poses of the n accepted particles, packed for one small device-to-host copy.
+__global__ void __launch_bounds__(256) k_gather_accepted(const uint32_t* __restrict__ list, uint32_t n, const float4* __restrict__ pos,
+                                                         const float4* __restrict__ quat, float4* __restrict__ pack) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint32_t pid = list[i];
+  pack[i] = pos[pid];
+  if (quat) pack[n + i] = quat[pid];
 }
 
 template <int SHAPE, bool CB>
@@ -396,6 +408,7 @@ __global__ void __launch_bounds__(MOVE_WARPS * 32) k_move(const MoveArgs A) {
         float4 pn = A.pos[pid];
         pn.x = r1.x; pn.y = r1.y; pn.z = r1.z;
         A.pos[pid] = pn;
+        if (A.acc_list) A.acc_list[atomicAdd(A.acc_count, 1u)] = pid;
         A.cpos[slot] = make_float4(r1.x, r1.y, r1.z, p0.w);
         if (SHAPE != SH_SPHERE && rot) {
           A.quat[pid] = as_f4(q1);

@@ -760,6 +760,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
         float4 pn = A.pos[pid];
         pn.x = r1f.x; pn.y = r1f.y; pn.z = r1f.z;
         A.pos[pid] = pn;
+        if (A.acc_list) A.acc_list[atomicAdd(A.acc_count, 1u)] = pid;
         A.cpos[slot] = make_float4(r1f.x, r1f.y, r1f.z, __uint_as_float(pid));
         if (ANISO && rot) {
           A.quat[pid] = s_q1[e];

@@ -319,21 +319,38 @@ def test_error_codes():
     h.close()
 
 
-def test_host_buffer_step_matches_device_path():
-    """hpmc_step_host (library-owned buffers, host<->device copies inside) gives the same bits."""
+@pytest.mark.parametrize("name,N,n_R_scale", [("C1", None, 1.0), ("C4", 4096, 1.0), ("C4", 4096, 0.0), ("C5", 512, 1.0), ("C7", 4096, 1.0)])
+def test_host_buffer_step_matches_device_path(name, N, n_R_scale):
+    """hpmc_step_host (library-owned buffers, host<->device copies inside) gives the same bits in the host arrays,
+    through the sparse download (few accepted particles: only their poses come back and are patched in) and the full
+    one (C4 without depletants: more than N/4 particles accepted per sweep)."""
     import torch
     import paper_1508_07077_b200 as hp
-    cfg = workloads.config("C1")
-    pos, _ = workloads.generate(cfg)
-    o, h, dpos, _ = _mk(cfg, pos, None)
-    hh = hp.HPMC(cfg.shape, cfg.sigma_c, cfg.sigma_d, cfg.box_L, cfg.d_max, None, None, N=cfg.N)
+    cfg = workloads.config(name, N)
+    pos, quat = workloads.generate(cfg)
+    o, h, dpos, _ = _mk(cfg, pos, quat)
+    hh = hp.HPMC(cfg.shape, cfg.sigma_c, cfg.sigma_d, cfg.box_L, cfg.d_max, None, None, cfg.disk_a, cfg.disk_s, N=cfg.N)
     hpos = torch.from_numpy(pos.copy()).pin_memory()
+    hquat = None if quat is None else torch.from_numpy(quat.copy()).pin_memory()
     hout = torch.zeros(cfg.N, dtype=torch.uint8).pin_memory()
-    for s in range(5):
-        o.build_cells(1, s); o.sweep(1, s, cfg.n_R(), cfg.d_max)
-        hh.step_host(hpos, None, hout, 1, s, cfg.n_R(), cfg.d_max)
+    n_R = cfg.n_R() * n_R_scale
+    full = 16 * cfg.N * (1 if quat is None else 2)
+    sparse_seen = full_seen = False
+    for s in range(8):
+        o.build_cells(1, s); o.sweep(1, s, n_R, cfg.d_max, cfg.a_max, cfg.n_trial)
+        hh.step_host(hpos, hquat, hout, 1, s, n_R, cfg.d_max, cfg.a_max, cfg.n_trial)
         assert np.array_equal(hout.numpy(), o.outcomes())
         assert np.array_equal(_bits(hpos.numpy()), _bits(o.pos))
+        if quat is not None:
+            assert np.array_equal(_bits(hquat.numpy()), _bits(o.quat))
+        h2d, d2h = hh.step_host_bytes()
+        assert h2d == full
+        nacc = int((o.outcomes() == 1).sum())
+        if nacc <= cfg.N // 4:
+            assert d2h == cfg.N + 4 + nacc * (4 + full // cfg.N); sparse_seen = True
+        else:
+            assert d2h == cfg.N + 4 + full; full_seen = True
+    assert full_seen if n_R_scale == 0.0 else sparse_seen
     hh.close(); h.close()
 
 
