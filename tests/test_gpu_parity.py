@@ -245,6 +245,19 @@ def test_c7_tetrahedra(monkeypatch, n_trial, kernel, options, N, sweeps):
         h.close()
 
 
+@pytest.mark.parametrize("name,N,options", [("C1", None, 0), ("C3", 16384, 1), ("C4", 4096, 0), ("C5", 512, 0), ("C6", 4096, 0),
+                                            ("C7", 4096, 1)])
+def test_warp_per_cell_kernel_plain_rule(monkeypatch, name, N, options):
+    """HPMC_MOVE_KERNEL=warp: the first kernel design (one warp per active cell, 32 depletants per step, ballot exit;
+    north_star's sketch) on every shape, plain rule, with and without the shell option: same bits as the oracle."""
+    import dataclasses
+    monkeypatch.setenv("HPMC_MOVE_KERNEL", "warp")
+    cfg = dataclasses.replace(workloads.config(name, N), n_trial=0)
+    pos, quat = workloads.generate(cfg)
+    c = run_parity(cfg, pos, quat, 40 if FULL else 10, cfg.n_R(), options=options)
+    assert c["rej_depletant"] > 0
+
+
 def test_one_launch_per_pass_mode(monkeypatch):
     """HPMC_SWEEP_LAUNCHES=8: the item-queue kernel launched once per checkerboard pass (no neighbour waits) instead of
     once per sweep; same bits."""
