@@ -108,6 +108,17 @@ def test_c3_spheres_full_size():
     assert c["dep_drawn"] > 2000 * (c["trials_trans"] - c["rej_boundary"] - c["rej_hard"])
 
 
+def test_spheres_beyond_one_wave_4m():
+    """Four times configs[2]: 4,194,304 spheres at C3's densities (178^3 cells) need more CTAs than the device holds at
+    once, so the sweep falls back to one launch per pass (3874 CTAs); two sweeps, bit for bit."""
+    if not FULL:
+        pytest.skip("long: 25 s of input placement")
+    cfg = workloads.config("C3", 4194304)
+    pos, _ = workloads.generate(cfg)
+    c = run_parity(cfg, pos, None, 2, cfg.n_R(), check_cells_every=1)
+    assert c["trials_trans"] > 3000000
+
+
 def test_c3_small_steps_accepting_moves_use_all_depletants():
     """Accepted moves at C3's density must test all ~2.8k depletants: tiny steps make acceptance common."""
     import dataclasses
