@@ -200,7 +200,45 @@ typedef struct {
 } hpmc_alu_peaks_t;
 int hpmc_alu_peaks(hpmc_alu_peaks_t* out, void* cuda_stream);
 
-/* Message of the last error on this context (or of the last failed hpmc_init if ctx is NULL). */
+/* Cell-list build without any device allocation (step a2 on its own).
+ *
+ * Who this is for.  Every other call needs an hpmc_ctx, and hpmc_init / hpmc_free_volume / hpmc_step_host obtain their
+ * working buffers with cudaMalloc.  Some programs that want the checkerboard cell list of a configuration cannot afford
+ * that: an analysis hook (cluster search, local density, neighbour query) called from inside a running simulation
+ * whose framework pool -- PyTorch's caching allocator, a simulation engine's arena -- already owns almost all of HBM, so
+ * that a raw cudaMalloc from this library fails although the application has memory to spare; and per-step code for
+ * which cudaMalloc / cudaFree are too costly because cudaFree waits for every stream of the device.  For them this one
+ * entry point keeps its working storage (cell counts, scan partials, per-particle cell id and rank) in a fixed array
+ * that is part of the library image: 3 MiB that every GPU which loads the library holds until the process exits.  It
+ * calls no cudaMalloc, cudaFree or other allocating routine, creates no context and needs none.
+ *
+ *   d_pos4        device, N x float4 centres (x, y, z, unused), 0 <= x,y,z < box_L; read only
+ *   N             1 .. 262,144                                  } beyond either limit: HPMC_E_BADARG, nothing is launched;
+ *   n_c           cells per axis, 1 .. 64 (n_c^3 <= 262,144)    } hpmc_last_error(NULL) names the limit
+ *   box_L         edge of the cubic periodic box; cell width w = box_L / n_c in fp32, as hpmc_init computes it
+ *   host_shift3   host, 3 floats in [0, box_L]: the grid shift (hpmc_build_cells draws it from Philox(seed, step) and
+ *                 hpmc_cells reports it; pass zeros for an unshifted grid)
+ *   d_cell_start  device, n_c^3 + 1 uint32, caller-owned, written: first slot of every cell, cells in ascending linear
+ *                 index (ix fastest); d_cell_start[n_c^3] = N
+ *   d_cell_pid    device, N uint32, caller-owned, written: particle ids, ascending inside each cell
+ *   cuda_stream   a cudaStream_t or NULL; the work is enqueued there and the call returns without synchronising
+ * The result equals, bit for bit, what hpmc_build_cells + hpmc_cells give for the same poses, grid and shift.
+ *
+ * Rules that follow from the shared array:
+ *   - One array per GPU serves every call, whatever the stream or thread.  Two calls whose kernels can overlap on the
+ *     GPU (different streams, no event between them) race on it and both results are garbage; calls on one stream, or
+ *     ordered by events, are fine.  The array keeps the previous call's contents; the part that must start at zero is
+ *     cleared (cudaMemsetAsync on the same stream) at the start of every call, so nothing carries over.
+ *   - The first call on each device looks up the array's device address (cudaGetSymbolAddress, with that device
+ *     current) and remembers it; later calls on that device skip this.  Make that first call before any stream
+ *     capture is begun.  Call with the device current that owns d_pos4 and the outputs.
+ * Errors: HPMC_E_BADARG (NULL pointer, sizes beyond the limits above, box_L <= 0, shift outside [0, box_L]),
+ * HPMC_E_CUDA (no device, address look-up or launch failure); message in hpmc_last_error(NULL). */
+int hpmc_cells_noalloc(const float* d_pos4, int64_t N, float box_L, int32_t n_c, const float* host_shift3,
+                       uint32_t* d_cell_start, uint32_t* d_cell_pid, void* cuda_stream);
+
+/* Message of the last error on this context (or, if ctx is NULL, of the last failed call that takes no context --
+ * hpmc_init, hpmc_alu_peaks, hpmc_cells_noalloc -- on the calling thread). */
 const char* hpmc_last_error(hpmc_ctx* ctx);
 
 #ifdef __cplusplus

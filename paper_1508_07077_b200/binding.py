@@ -22,7 +22,7 @@ EXPORTS = (
     "hpmc_init", "hpmc_destroy", "hpmc_build_cells", "hpmc_sweep", "hpmc_run", "hpmc_counters",
     "hpmc_reset_counters", "hpmc_outcomes", "hpmc_grid", "hpmc_cells", "hpmc_upload", "hpmc_download",
     "hpmc_step_host", "hpmc_launch_count", "hpmc_time_move_kernel", "hpmc_move_kernel_ms", "hpmc_last_error",
-    "hpmc_alu_peaks", "hpmc_set_options", "hpmc_free_volume", "hpmc_step_host_bytes",
+    "hpmc_alu_peaks", "hpmc_set_options", "hpmc_free_volume", "hpmc_step_host_bytes", "hpmc_cells_noalloc",
 )
 
 
@@ -92,6 +92,7 @@ def load_library() -> C.CDLL:
         "hpmc_move_kernel_ms": (i32, [vp, P(f64), P(i64)]),
         "hpmc_last_error": (C.c_char_p, [vp]),
         "hpmc_alu_peaks": (i32, [P(AluPeaks), vp]),
+        "hpmc_cells_noalloc": (i32, [vp, i64, f32, i32, P(f32 * 3), vp, vp, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -117,6 +118,27 @@ def alu_peaks(stream=None):
 
 def _dptr(t):
     return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def cells_noalloc(pos4, box_L, n_c, shift3, cell_start, cell_pid, stream=None):
+    """hpmc_cells_noalloc: the checkerboard cell list of `pos4` written into the caller's `cell_start` (n_c^3 + 1 int32)
+    and `cell_pid` (N int32) CUDA tensors, with no device allocation inside the library -- for callers whose memory pool
+    owns the GPU or who cannot pay for cudaMalloc / cudaFree in their loop (include/hpmc.h has the whole contract: at most
+    262,144 particles and n_c <= 64, one shared scratch array per GPU, so calls that overlap on the GPU race).
+    Asynchronous on `stream` (default: torch's current stream); the three tensors must stay alive until it has run."""
+    import torch
+    L = load_library()
+    s = torch.cuda.current_stream() if stream is None else stream
+    for t in (pos4, cell_start, cell_pid):
+        assert t.is_cuda and t.is_contiguous()
+    assert pos4.dtype == torch.float32 and pos4.shape[1] == 4
+    assert cell_start.dtype == torch.int32 and cell_pid.dtype == torch.int32
+    assert cell_pid.numel() >= pos4.shape[0] and cell_start.numel() >= int(n_c) ** 3 + 1
+    sh = (C.c_float * 3)(*[float(x) for x in shift3])
+    rc = L.hpmc_cells_noalloc(_dptr(pos4), int(pos4.shape[0]), float(box_L), int(n_c), C.byref(sh), _dptr(cell_start),
+                              _dptr(cell_pid), C.c_void_p(s.cuda_stream))
+    if rc:
+        raise HPMCError(rc, (L.hpmc_last_error(None) or b"").decode())
 
 
 class HPMC:

@@ -13,6 +13,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <algorithm>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -888,3 +889,159 @@ int hpmc_alu_peaks(hpmc_alu_peaks_t* out, void* cuda_stream) {
 const char* hpmc_last_error(hpmc_ctx* ctx) { return ctx ? ctx->err.c_str() : g_init_error.c_str(); }
 
 }  // extern "C"
+
+// =====================================================================================================================
+// hpmc_cells_noalloc: step a2 (cell-list build) for callers that may not allocate device memory.
+// Contract and rationale: include/hpmc.h.  Nothing above this line is touched by it; the kernels it shares with
+// hpmc_build_cells (k_scan_tiles, k_fill, the device helpers of cells.cuh) are used as they are, through pointers.
+//
+// The working storage of the build (per-cell counts, scan tile totals, per-particle cell id and arrival rank) lives in
+// ONE file-scope device array of fixed size instead of cudaMalloc'ed buffers.  Layout in 32-bit words:
+//   [0, NA_MAX_CELLS)                 counts     must be zero when k_na_bin starts: cleared at the top of every call
+//   [.., + NA_MAX_TILES)              tile_sums  fully rewritten by k_scan_tiles before it is read
+//   [.., + NA_MAX_N)                  cid        rewritten for i < N before it is read
+//   [.., + NA_MAX_N)                  rank       likewise
+// 3 MiB + 512 B, present on every GPU that loads the library, for the life of the process.
+// =====================================================================================================================
+
+namespace {
+constexpr int NA_MAX_N = 1 << 18;                         // 262,144 particles
+constexpr int NA_MAX_CELLS = 1 << 18;                     // 262,144 cells, i.e. n_c <= 64
+constexpr int NA_MAX_TILES = NA_MAX_CELLS / SCAN_TILE;
+static_assert(NA_MAX_CELLS % SCAN_TILE == 0, "the counts region is scanned in whole tiles");
+constexpr size_t NA_OFF_COUNTS = 0;
+constexpr size_t NA_OFF_TILES = NA_OFF_COUNTS + NA_MAX_CELLS;
+constexpr size_t NA_OFF_CID = NA_OFF_TILES + NA_MAX_TILES;
+constexpr size_t NA_OFF_RANK = NA_OFF_CID + NA_MAX_N;
+constexpr size_t NA_WORDS = NA_OFF_RANK + NA_MAX_N;
+static_assert(NA_OFF_TILES % 64 == 0 && NA_OFF_CID % 64 == 0 && NA_OFF_RANK % 64 == 0, "sub-arrays stay 256-byte aligned");
+}  // namespace
+
+// In host code this name is only a handle for cudaGetSymbolAddress -- it is NOT a device pointer and must never be
+// handed to a kernel or to cudaMemset* as one.  na_scratch_of_current_device() below turns it into the real address.
+static __device__ __align__(256) uint32_t g_na_scratch[NA_WORDS];
+
+namespace {
+
+// k_bin_count without the outcome-code reset (there is no sweep behind this build) and with the cell index clamped at
+// zero, so that a pose outside [0, L) -- a caller error -- lands in an edge cell instead of writing out of bounds.
+__global__ void __launch_bounds__(256) k_na_bin(const float4* __restrict__ pos, int N, Geo g, float sx, float sy, float sz,
+                                                uint32_t* __restrict__ cid, uint32_t* __restrict__ rank,
+                                                uint32_t* __restrict__ counts) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= N) return;
+  const float4 p = pos[i];
+  const int ix = max(cell_axis(g, p.x, sx), 0), iy = max(cell_axis(g, p.y, sy), 0), iz = max(cell_axis(g, p.z, sz), 0);
+  const uint32_t c = ((uint32_t)iz * g.nc + iy) * g.nc + ix;
+  cid[i] = c;
+  rank[i] = atomicAdd(&counts[c], 1u);
+}
+
+// k_scan_apply<true> writing into a caller-owned cell_start of exactly n + 1 words (no padding to write into, so the
+// stores are guarded scalars) and leaving the counts alone (the next call clears them itself).
+__global__ void __launch_bounds__(SCAN_THREADS) k_na_scan_apply(const uint32_t* __restrict__ counts, int n,
+                                                                const uint32_t* __restrict__ tile_sums,
+                                                                uint32_t* __restrict__ cell_start) {
+  __shared__ uint32_t s_warp[32];
+  __shared__ uint32_t s_off;
+  uint32_t part = 0;
+  for (int i = threadIdx.x; i < (int)blockIdx.x; i += SCAN_THREADS) part += tile_sums[i];
+  uint32_t tot;
+  block_exclusive_scan(part, s_warp, tot);
+  if (threadIdx.x == 0) s_off = tot;
+  __syncthreads();
+  const uint32_t off = s_off;
+  const int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+  uint32_t v[SCAN_ITEMS], s = 0;
+  load8(counts + base, v);                         // the words between n and the end of the last tile are zero
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) s += v[k];
+  uint32_t total;
+  uint32_t run = off + block_exclusive_scan(s, s_warp, total);
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) {
+    if (base + k <= n) cell_start[base + k] = run;   // index n receives the grand total N
+    run += v[k];
+  }
+  if (base + SCAN_ITEMS == n) cell_start[n] = run;   // n a whole number of tiles: nobody owns index n above
+}
+
+// the ordering half of k_sort_write: ascending particle id inside every cell (undoes the atomics' arrival order)
+__global__ void __launch_bounds__(256) k_na_sort(const uint32_t* __restrict__ cell_start, int ncell,
+                                                 uint32_t* __restrict__ cell_pid) {
+  const int c = blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= ncell) return;
+  const uint32_t b = cell_start[c], e = cell_start[c + 1];
+  for (uint32_t s = b + 1; s < e; ++s) {
+    const uint32_t v = cell_pid[s];
+    uint32_t t = s;
+    while (t > b && cell_pid[t - 1] > v) { cell_pid[t] = cell_pid[t - 1]; --t; }
+    cell_pid[t] = v;
+  }
+}
+
+constexpr int NA_MAX_DEVICES = 64;
+std::mutex g_na_mutex;
+uint32_t* g_na_dev_ptr[NA_MAX_DEVICES] = {};     // device address of g_na_scratch, one per device, filled on first use
+
+// Set-up, once per device, with that device current: ask the runtime where g_na_scratch lives on THIS device.
+int na_scratch_of_current_device(uint32_t** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess)
+    return fail(nullptr, HPMC_E_CUDA, std::string("hpmc_cells_noalloc: no usable CUDA device: ") + cudaGetErrorString(e));
+  if (dev < 0 || dev >= NA_MAX_DEVICES) return fail(nullptr, HPMC_E_CUDA, "hpmc_cells_noalloc: device ordinal beyond 63");
+  std::lock_guard<std::mutex> lock(g_na_mutex);
+  if (!g_na_dev_ptr[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_na_scratch);
+    if (e != cudaSuccess || !p)
+      return fail(nullptr, HPMC_E_CUDA, std::string("hpmc_cells_noalloc: cudaGetSymbolAddress(g_na_scratch): ") + cudaGetErrorString(e));
+    g_na_dev_ptr[dev] = static_cast<uint32_t*>(p);
+  }
+  *out = g_na_dev_ptr[dev];
+  return HPMC_OK;
+}
+
+}  // namespace
+
+extern "C" int hpmc_cells_noalloc(const float* d_pos4, int64_t N, float box_L, int32_t n_c, const float* host_shift3,
+                                  uint32_t* d_cell_start, uint32_t* d_cell_pid, void* cuda_stream) {
+  hpmc_ctx* ctx = nullptr;                          // CU() reports through hpmc_last_error(NULL)
+  if (!d_pos4 || !host_shift3 || !d_cell_start || !d_cell_pid)
+    return fail(nullptr, HPMC_E_BADARG, "hpmc_cells_noalloc: NULL argument");
+  if (N < 1 || N > NA_MAX_N)
+    return fail(nullptr, HPMC_E_BADARG, "hpmc_cells_noalloc: N = " + std::to_string(N) + " is outside 1 .. " +
+                                            std::to_string(NA_MAX_N) + " (the fixed scratch array holds no more; use "
+                                            "hpmc_init + hpmc_build_cells for larger systems)");
+  if (n_c < 1 || (int64_t)n_c * n_c * n_c > NA_MAX_CELLS)
+    return fail(nullptr, HPMC_E_BADARG, "hpmc_cells_noalloc: n_c = " + std::to_string(n_c) + " is outside 1 .. 64 (n_c^3 <= " +
+                                            std::to_string(NA_MAX_CELLS) + " cells fit the fixed scratch array)");
+  if (!(box_L > 0.0f)) return fail(nullptr, HPMC_E_BADARG, "hpmc_cells_noalloc: box_L must be positive");
+  for (int a = 0; a < 3; ++a)
+    if (!(host_shift3[a] >= 0.0f && host_shift3[a] <= box_L))
+      return fail(nullptr, HPMC_E_BADARG, "hpmc_cells_noalloc: grid shift outside [0, box_L]");
+  uint32_t* scratch = nullptr;
+  const int rc = na_scratch_of_current_device(&scratch);
+  if (rc) return rc;
+  uint32_t* counts = scratch + NA_OFF_COUNTS;
+  uint32_t* tile_sums = scratch + NA_OFF_TILES;
+  uint32_t* cid = scratch + NA_OFF_CID;
+  uint32_t* rank = scratch + NA_OFF_RANK;
+
+  Geo g{};                                          // the binning reads L, w and nc only; same fp32 expressions as make_geo
+  g.L = box_L; g.halfL = 0.5f * box_L; g.nc = n_c; g.w = box_L / (float)n_c;
+  const int n = (int)N, ncell = n_c * n_c * n_c;
+  const int ntiles = (ncell + SCAN_TILE - 1) / SCAN_TILE, nb = (n + 255) / 256;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  // the array keeps whatever the previous call (any stream, any size) left in it: the counts must start at zero
+  CU(cudaMemsetAsync(counts, 0, sizeof(uint32_t) * (size_t)ntiles * SCAN_TILE, st));
+  k_na_bin<<<nb, 256, 0, st>>>(reinterpret_cast<const float4*>(d_pos4), n, g, host_shift3[0], host_shift3[1],
+                               host_shift3[2], cid, rank, counts);
+  k_scan_tiles<<<ntiles, SCAN_THREADS, 0, st>>>(counts, ncell, tile_sums);
+  k_na_scan_apply<<<ntiles, SCAN_THREADS, 0, st>>>(counts, ncell, tile_sums, d_cell_start);
+  k_fill<<<nb, 256, 0, st>>>(cid, rank, d_cell_start, n, d_cell_pid);
+  k_na_sort<<<(ncell + 255) / 256, 256, 0, st>>>(d_cell_start, ncell, d_cell_pid);
+  CU(cudaGetLastError());
+  return HPMC_OK;
+}
