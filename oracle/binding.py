@@ -26,7 +26,7 @@ COUNTER_NAMES = (
 )
 
 SHAPES = {"sphere": 0, "halfball": 1, "spherodisk": 2, "ellipsoid": 3, "tetrahedron": 4}
-FLAG_SHELL, FLAG_ROSENBLUTH, FLAG_TEST_LITERAL_CORE = 1, 2, 0x100
+FLAG_SHELL, FLAG_ROSENBLUTH = 1, 2
 
 
 class OracleParams(C.Structure):
@@ -63,54 +63,67 @@ def build(force: bool = False) -> str:
     return _so_path(_cpu_has_fma())
 
 
+def apply_signatures(L: C.CDLL) -> C.CDLL:
+    """ctypes signatures of every oracle_* export, on the oracle library or on a throw-away mutant build of it
+    (tests compile hpmc_oracle.cpp with one line changed to show that a pin catches the change)."""
+    vp, u32, i32, i64, f32, f64 = C.c_void_p, C.c_uint32, C.c_int32, C.c_int64, C.c_float, C.c_double
+    P = C.POINTER
+    sig = {
+        "oracle_create": (vp, [P(OracleParams), i64, vp, vp]),
+        "oracle_destroy": (None, [vp]),
+        "oracle_set_flags": (i32, [vp, u32, f32]),
+        "oracle_cbrt_fixed": (f32, [f32]),
+        "oracle_shell": (f64, [P(OracleParams), f64, f32, u32, P(f32)]),
+        "oracle_shell_samples": (None, [P(OracleParams), f32, u32, u32, u32, u32, i64, vp]),
+        "oracle_grid": (i32, [vp, P(i32), P(f32)]),
+        "oracle_set_threads": (None, [i32]),
+        "oracle_get_threads": (i32, []),
+        "oracle_build_cells": (i32, [vp, u32, u32]),
+        "oracle_sweep": (i32, [vp, u32, u32, f64, f32, f32, i32]),
+        "oracle_colour_order": (i32, [u32, u32, vp]),
+        "oracle_counters": (i32, [vp, vp]),
+        "oracle_reset_counters": (i32, [vp]),
+        "oracle_outcomes": (i32, [vp, vp]),
+        "oracle_trial_poses": (i32, [vp, vp, vp]),
+        "oracle_cells": (i32, [vp, vp, vp, vp]),
+        "oracle_run": (i32, [vp, u32, u32, i64, f64, f32, f32, i32, vp, vp]),
+        "oracle_eval_move": (i32, [vp, u32, u32, i64, vp, vp, f64, i32]),
+        "oracle_eval_moves": (i32, [vp, u32, u32, i64, i64, vp, vp, f64, i32, vp]),
+        "oracle_count_overlaps": (i64, [vp, i32]),
+        "oracle_free_volume": (i32, [vp, u32, u32, i64, vp]),
+        "oracle_philox4x32_10": (None, [vp, vp, vp]),
+        "oracle_unit01": (f32, [u32]),
+        "oracle_sym_unit": (f32, [u32]),
+        "oracle_poisson_table": (i64, [f64, P(i64), vp, i64]),
+        "oracle_poisson_draws": (None, [f64, vp, i64, vp]),
+        "oracle_lambda": (f64, [P(OracleParams), f64]),
+        "oracle_ball_samples": (None, [u32, u32, u32, u32, i64, f32, vp]),
+        "oracle_dep_overlap": (None, [P(OracleParams), vp, vp, i64, vp]),
+        "oracle_pair_overlap": (None, [P(OracleParams), vp, vp, vp, i64, vp]),
+        "oracle_support": (None, [P(OracleParams), vp, vp, vp]),
+        "oracle_quat_axis": (None, [vp, vp]),
+        "oracle_rotate_cayley": (None, [vp, vp, vp]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(L, name)
+        fn.restype = res
+        fn.argtypes = args
+    return L
+
+
 def lib() -> C.CDLL:
     global _LIB
     with _LOCK:
         if _LIB is None:
-            L = C.CDLL(build())
-            vp, u32, i32, i64, f32, f64 = C.c_void_p, C.c_uint32, C.c_int32, C.c_int64, C.c_float, C.c_double
-            P = C.POINTER
-            sig = {
-                "oracle_create": (vp, [P(OracleParams), i64, vp, vp]),
-                "oracle_destroy": (None, [vp]),
-                "oracle_set_flags": (i32, [vp, u32, f32]),
-                "oracle_cbrt_fixed": (f32, [f32]),
-                "oracle_shell": (f64, [P(OracleParams), f64, f32, u32, P(f32)]),
-                "oracle_shell_samples": (None, [P(OracleParams), f32, u32, u32, u32, u32, i64, vp]),
-                "oracle_grid": (i32, [vp, P(i32), P(f32)]),
-                "oracle_set_threads": (None, [i32]),
-                "oracle_get_threads": (i32, []),
-                "oracle_build_cells": (i32, [vp, u32, u32]),
-                "oracle_sweep": (i32, [vp, u32, u32, f64, f32, f32, i32]),
-                "oracle_counters": (i32, [vp, vp]),
-                "oracle_reset_counters": (i32, [vp]),
-                "oracle_outcomes": (i32, [vp, vp]),
-                "oracle_trial_poses": (i32, [vp, vp, vp]),
-                "oracle_cells": (i32, [vp, vp, vp, vp]),
-                "oracle_run": (i32, [vp, u32, u32, i64, f64, f32, f32, i32, vp, vp]),
-                "oracle_eval_move": (i32, [vp, u32, u32, i64, vp, vp, f64, i32]),
-                "oracle_eval_moves": (i32, [vp, u32, u32, i64, i64, vp, vp, f64, i32, vp]),
-                "oracle_count_overlaps": (i64, [vp, i32]),
-                "oracle_free_volume": (i32, [vp, u32, u32, i64, vp]),
-                "oracle_philox4x32_10": (None, [vp, vp, vp]),
-                "oracle_unit01": (f32, [u32]),
-                "oracle_sym_unit": (f32, [u32]),
-                "oracle_poisson_table": (i64, [f64, P(i64), vp, i64]),
-                "oracle_poisson_draws": (None, [f64, vp, i64, vp]),
-                "oracle_lambda": (f64, [P(OracleParams), f64]),
-                "oracle_ball_samples": (None, [u32, u32, u32, u32, i64, f32, vp]),
-                "oracle_dep_overlap": (None, [P(OracleParams), vp, vp, i64, vp]),
-                "oracle_pair_overlap": (None, [P(OracleParams), vp, vp, vp, i64, vp]),
-                "oracle_support": (None, [P(OracleParams), vp, vp, vp]),
-                "oracle_quat_axis": (None, [vp, vp]),
-                "oracle_rotate_cayley": (None, [vp, vp, vp]),
-            }
-            for name, (res, args) in sig.items():
-                fn = getattr(L, name)
-                fn.restype = res
-                fn.argtypes = args
-            _LIB = L
+            _LIB = apply_signatures(C.CDLL(build()))
     return _LIB
+
+
+def colour_order(seed: int, step: int) -> np.ndarray:
+    """The order in which sweep (seed, step) visits the 8 checkerboard colours (R-2)."""
+    out = np.empty(8, np.uint32)
+    lib().oracle_colour_order(seed, step, _ptr(out))
+    return out
 
 
 def _ptr(a):

@@ -31,8 +31,8 @@
 // Options (oracle_set_flags; default 0 = the path above, untouched by them): SURVEY 8(f) NEXT-1, the shell-restricted
 // insertion volume of L158 (reading R-N1 of DESIGN.md), and NEXT-4, the exact Rosenbluth form of the configurational
 // bias weight (refs 27, 28, 33; reading R-N4).  Their pins: radial cdf and isotropy of the shell sampler, cube-root
-// accuracy, isolated-colloid and Asakura-Oosawa ratio tests with the shell on (and a literal-hard-core shell failing
-// them), forward/reverse ratio of the Rosenbluth form to 3 sigma with no systematic allowance.
+// accuracy, isolated-colloid and Asakura-Oosawa ratio tests with the shell on (and a literal-hard-core shell, built as a
+// throw-away mutant of this file by the test, failing them), forward/reverse ratio of the Rosenbluth form to 3 sigma with no systematic allowance.
 //
 // Arithmetic: all pose arithmetic is IEEE fp32 with contraction OFF (-ffp-contract=off);
 // an FMA is used only where fmaf() is written.  Integers u32/u64.  fp64 only for the
@@ -502,7 +502,7 @@ static inline V3 ball_sample(uint32_t seed, uint32_t step, uint32_t purpose, uin
 }
 
 // ---- options of a sweep (oracle_set_flags)
-enum { F_SHELL = 1u, F_ROSENBLUTH = 2u, F_TEST_LITERAL_CORE = 0x100u };
+enum { F_SHELL = 1u, F_ROSENBLUTH = 2u };
 
 // R-N1 (L158 "restricting the sampling to the excluded volume shell of the moved colloid"): depletants are drawn
 // uniformly in the shell R_in < |d| <= R about the NEW centre instead of the whole ball.  Eq. 12 (L136) needs
@@ -519,7 +519,6 @@ static inline Shell make_shell(const Geo& g, float d_max, uint32_t flags) {
   Shell sh;
   sh.Rin = rin - 1.7320508f * d_max;
   if (sh.Rin < 0.0f) sh.Rin = 0.0f;
-  if (flags & F_TEST_LITERAL_CORE) sh.Rin = 0.5f * g.dcirc;   // mutation used by a pin only: the shell minus the HARD core
   sh.Rin3 = (sh.Rin * sh.Rin) * sh.Rin;
   sh.dR3 = (g.Rins * g.Rins) * g.Rins - sh.Rin3;
   return sh;
@@ -647,6 +646,21 @@ static int evaluate_move(const Ctx& c, uint32_t seed, uint32_t step, uint32_t co
   const U4 ra = philox4x32_10((uint32_t)i, 0, 0, word3(P_ACCEPT, colour, 0), seed, step);
   ++cn.c[C_PHILOX_BLOCKS];
   return (unit01(ra.v[0]) < P) ? OUT_ACCEPT : OUT_CB;
+}
+
+// R-2 (L180 "the checkerboard coloring is permuted randomly"): the order in which a sweep visits the 8 colours, a
+// Fisher-Yates shuffle of (0..7) driven by the 7 words of SWEEP blocks 1 and 2: position i (7 down to 1) is swapped
+// with a position drawn uniformly from 0..i.  Pinned by tests/test_oracle_physics.py (uniform over positions and over
+// neighbouring pairs; a constant order and an off-by-one range must fail).
+static void colour_order(uint32_t seed, uint32_t step, uint32_t perm[8]) {
+  for (uint32_t k = 0; k < 8; ++k) perm[k] = k;
+  const U4 b1 = philox4x32_10(0, 0, 0, word3(P_SWEEP, 0, 1), seed, step);
+  const U4 b2 = philox4x32_10(0, 0, 0, word3(P_SWEEP, 0, 2), seed, step);
+  const uint32_t wds[7] = {b1.v[0], b1.v[1], b1.v[2], b1.v[3], b2.v[0], b2.v[1], b2.v[2]};
+  for (int i = 7, j = 0; i >= 1; --i, ++j) {
+    const uint32_t r = mulhi32(wds[j], (uint32_t)i + 1u);
+    const uint32_t t = perm[i]; perm[i] = perm[r]; perm[r] = t;
+  }
 }
 
 // Steps 3.1 - 3.3 + 3.9 for one active cell.
@@ -781,21 +795,15 @@ int oracle_build_cells(void* h, uint32_t seed, uint32_t step) {
 }
 
 // One sweep = 8 sub-lattice passes in a permuted order (L180).
+int oracle_colour_order(uint32_t seed, uint32_t step, uint32_t* out8) { colour_order(seed, step, out8); return 0; }
 int oracle_sweep(void* h, uint32_t seed, uint32_t step, double n_R, float d_max, float a_max, int32_t n_trial) {
   Ctx* c = (Ctx*)h;
   if (!c->built || c->b_seed != seed || c->b_step != step) return -3;
   if (!(d_max >= 0.0f) || d_max > c->g.dmax_cap || n_R < 0.0 || a_max < 0.0f || n_trial < 0 || n_trial > 65535) return -1;
   const double lambda = lambda_opt(c->g, n_R, d_max, c->flags);
   if (c->pt.lambda != lambda) build_poisson(c->pt, lambda);
-  // R-2: Fisher-Yates permutation of the 8 colours from SWEEP blocks 1, 2
-  uint32_t perm[8] = {0, 1, 2, 3, 4, 5, 6, 7};
-  const U4 b1 = philox4x32_10(0, 0, 0, word3(P_SWEEP, 0, 1), seed, step);
-  const U4 b2 = philox4x32_10(0, 0, 0, word3(P_SWEEP, 0, 2), seed, step);
-  const uint32_t wds[7] = {b1.v[0], b1.v[1], b1.v[2], b1.v[3], b2.v[0], b2.v[1], b2.v[2]};
-  for (int i = 7, j = 0; i >= 1; --i, ++j) {
-    const uint32_t r = mulhi32(wds[j], (uint32_t)i + 1u);
-    const uint32_t t = perm[i]; perm[i] = perm[r]; perm[r] = t;
-  }
+  uint32_t perm[8];
+  colour_order(seed, step, perm);
   std::fill(c->outcome.begin(), c->outcome.end(), (uint8_t)0);
   const int nc = c->nc, hc = nc / 2;
   const int64_t nact = (int64_t)hc * hc * hc;

@@ -55,7 +55,8 @@ def test_struct_layouts_match_header():
 
 def test_signatures_have_no_torch_types():
     src = open(HEADER).read()
-    assert "torch" not in src.lower().replace("torch.cuda.current_stream", "") or True
+    code = re.sub(r"/\*.*?\*/", " ", src, flags=re.S)          # comments may name torch (where a stream comes from)
+    assert "torch" not in code.lower()
     assert "at::" not in src and "c10::" not in src and "#include <torch" not in src
     assert 'extern "C"' in src
 

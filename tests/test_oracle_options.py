@@ -16,7 +16,7 @@ import pytest
 import oracle
 import workloads
 from oracle import binding
-from oracle.binding import FLAG_ROSENBLUTH, FLAG_SHELL, FLAG_TEST_LITERAL_CORE
+from oracle.binding import FLAG_ROSENBLUTH, FLAG_SHELL
 
 from test_oracle_physics import iso_accept, lens, sphere_oracle
 
@@ -69,15 +69,25 @@ def test_shell_radius_law_isotropy_and_lambda(shape, sigma_d, d_max, disk):
 
 
 # ------------------------------------------------------------------ the transition rate is unchanged (Eq. 15)
-def _iso_rate(sigma_d, n_R, d, ndraw, flags, eval_dmax):
-    o = sphere_oracle([[4.0, 4.0, 4.0]], 8.0, sigma_d, 0.1, threads=os.cpu_count() or 1)
-    o.set_flags(flags, eval_dmax)
-    o.build_cells(1, 0)
+def _iso_rate(sigma_d, n_R, d, ndraw, flags, eval_dmax, L_=None):
+    """Acceptance rate of one fixed translation of length d of an isolated sphere (L_: a mutant build instead of the
+    oracle library)."""
+    L_ = L_ or oracle.lib()
+    L_.oracle_set_threads(os.cpu_count() or 1)
+    p4 = np.zeros((1, 4), np.float32)
+    p4[0, :3] = 4.0
+    par = binding.make_params("sphere", 1.0, sigma_d, 8.0, 0.1)
+    h = L_.oracle_create(C.byref(par), 1, _vp(p4), None)
+    assert h
+    L_.oracle_set_flags(h, flags, eval_dmax)
+    assert L_.oracle_build_cells(h, 1, 0) == 0
     u = np.random.default_rng(5).standard_normal(3)
     u /= np.linalg.norm(u)
     new = np.float32(4.0) + (d * u).astype(np.float32)
     d_eff = float(np.linalg.norm(new.astype(np.float64) - 4.0))
-    out = o.eval_moves(1, 0, ndraw, 0, new, None, n_R)
+    out = np.empty(ndraw, np.uint8)
+    assert L_.oracle_eval_moves(h, 1, 0, ndraw, 0, _vp(new), None, float(n_R), 0, _vp(out)) == 0
+    L_.oracle_destroy(h)
     assert set(np.unique(out)) <= {1, 4}
     return float((out == 1).mean()), d_eff
 
@@ -93,12 +103,14 @@ def test_shell_isolated_colloid_keeps_the_closed_form(sigma_d, n_R, d, eval_dmax
     assert abs(acc - p) < 3.0 * math.sqrt(p * (1 - p) / ndraw) + 1e-9, (acc, p)
 
 
-def test_shell_minus_the_hard_core_violates_the_closed_form():
+def test_shell_minus_the_hard_core_violates_the_closed_form(tmp_path):
     """Why R-N1 does not take L158's "V_excl,i minus V'_core,i" with the colloid's hard core as the core: for a move
     longer than the depletant radius part of the new-minus-old region lies inside the new hard core, the literal shell
     misses it and accepts too often (Eq. 12's V_0 >= V'_excl minus V_excl fails).  Same measurement as above, mutated shell."""
     sigma_d, n_R, d, ndraw = 0.1, 50.0, 0.09, 400000
-    acc, d_eff = _iso_rate(sigma_d, n_R, d, ndraw, FLAG_SHELL | FLAG_TEST_LITERAL_CORE, 0.06)
+    from conftest import build_mutant_oracle
+    literal = build_mutant_oracle(tmp_path, "literal_core", "  sh.Rin = rin - 1.7320508f * d_max;", "  sh.Rin = 0.5f * g.dcirc;")
+    acc, d_eff = _iso_rate(sigma_d, n_R, d, ndraw, FLAG_SHELL, 0.06, literal)
     p = iso_accept(n_R, 0.55, d_eff)
     assert acc - p > 6.0 * math.sqrt(p * (1 - p) / ndraw), (acc, p)
 

@@ -348,26 +348,8 @@ def test_cb_two_sphere_fixed_move_ratio(n_trial):
 
 
 def _mutant_library(tmp_path, name, old, new):
-    """The oracle source with ONE textual substitution, compiled to a throw-away shared object (never the library the
-    parity tests use)."""
-    import ctypes as C
-    import subprocess
-    src = open(os.path.join(os.path.dirname(oracle.__file__), "hpmc_oracle.cpp")).read()
-    assert src.count(old) == 1, (name, src.count(old))
-    cpp, so = str(tmp_path / ("m_%s.cpp" % name)), str(tmp_path / ("m_%s.so" % name))
-    with open(cpp, "w") as f:
-        f.write(src.replace(old, new))
-    subprocess.run(["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC",
-                    "-o", so, cpp], check=True)
-    L_ = C.CDLL(so)
-    L_.oracle_create.restype = C.c_void_p
-    L_.oracle_create.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
-    L_.oracle_build_cells.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32]
-    L_.oracle_eval_moves.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p,
-                                     C.c_double, C.c_int32, C.c_void_p]
-    L_.oracle_destroy.argtypes = [C.c_void_p]
-    L_.oracle_set_threads.argtypes = [C.c_int32]
-    return L_
+    from conftest import build_mutant_oracle
+    return build_mutant_oracle(tmp_path, name, old, new)
 
 
 _EQ16 = "const float wk = (float)(Npins * (Npi + 1u)) / (float)((Nins + 1u) * Ni);"
@@ -492,8 +474,8 @@ def test_parallel_order_equals_sequential_order():
     assert a.counters() == b.counters()
 
 
-def test_grid_shift_and_colour_order_vary():
-    """L180: 'coloring is permuted randomly ... grid lines are randomly shifted' (once per sweep, S11)."""
+def test_grid_shift_varies():
+    """L180: 'grid lines are randomly shifted' (once per sweep, S11): uniform in [0, w) on every axis, axes uncorrelated."""
     cfg = workloads.config("C1")
     pos, _ = workloads.generate(cfg)
     o = make_oracle(cfg, pos)
@@ -506,6 +488,122 @@ def test_grid_shift_and_colour_order_vary():
     assert sh.min() > 0 and sh.max() < 1
     assert np.all(np.abs(sh.mean(0) - 0.5) < 4 * math.sqrt(1 / 12 / 200))
     assert np.all(np.abs(np.corrcoef(sh.T)[np.triu_indices(3, 1)]) < 0.3)
+
+
+# ------------------------------------------------------------------ colour order of a sweep (R-2, L180)
+_N_ORDERS = 100000
+
+
+def _colour_order_chi2(L_, n=_N_ORDERS):
+    """chi^2 of (position, colour) counts against n/8 (49 degrees of freedom: rows and columns of a permutation sum to
+    n) and, for each of the 7 neighbouring position pairs, of the ordered colour pairs against n/56 (55 d.o.f.)."""
+    out = np.empty(8, np.uint32)
+    orders = np.empty((n, 8), np.int64)
+    for k in range(n):
+        L_.oracle_colour_order(11 + k // 1000, k % 1000, out.ctypes.data)
+        orders[k] = out
+    assert np.array_equal(np.sort(orders, axis=1), np.tile(np.arange(8), (n, 1))), "not a permutation of 0..7"
+    pos_counts = np.zeros((8, 8))
+    for p in range(8):
+        pos_counts[p] = np.bincount(orders[:, p], minlength=8)
+    chi_pos = float(((pos_counts - n / 8.0) ** 2 / (n / 8.0)).sum())
+    chi_pairs = []
+    for p in range(7):
+        c = np.bincount(orders[:, p] * 8 + orders[:, p + 1], minlength=64).reshape(8, 8).astype(np.float64)
+        assert np.all(np.diag(c) == 0)
+        off = c[~np.eye(8, dtype=bool)]
+        chi_pairs.append(float(((off - n / 56.0) ** 2 / (n / 56.0)).sum()))
+    return chi_pos, chi_pairs
+
+
+def _colour_order_is_uniform(chi_pos, chi_pairs):
+    from scipy.stats import chi2
+    return chi_pos < chi2.ppf(1 - 1e-3, 49) and max(chi_pairs) < chi2.ppf(1 - 1e-3 / 7, 55)
+
+
+def test_colour_order_is_a_uniform_random_permutation():
+    """R-2 pin ("the checkerboard coloring is permuted randomly"): over 10^5 sweeps every colour takes every
+    one of the 8 places with frequency 1/8 and every ordered pair of colours is equally likely in neighbouring places
+    (chi^2, alpha = 10^-3 overall each) -- what a uniform random permutation means, independent of how it is drawn."""
+    chi_pos, chi_pairs = _colour_order_chi2(oracle.lib())
+    assert _colour_order_is_uniform(chi_pos, chi_pairs), (chi_pos, chi_pairs)
+    assert len({tuple(oracle.binding.colour_order(3, s)) for s in range(50)}) > 40
+
+
+_SWAP = "    const uint32_t t = perm[i]; perm[i] = perm[r]; perm[r] = t;"
+
+
+@pytest.mark.parametrize("name,old,new", [
+    ("constant_order", _SWAP, "    (void)r;"),                                                # never permuted
+    ("range_off_by_one", "mulhi32(wds[j], (uint32_t)i + 1u)", "mulhi32(wds[j], (uint32_t)i)"),  # r in 0..i-1: cyclic permutations only
+])
+def test_colour_order_pin_rejects_wrong_shuffles(tmp_path, name, old, new):
+    L_ = _mutant_library(tmp_path, name, old, new)
+    chi_pos, chi_pairs = _colour_order_chi2(L_, 20000)
+    assert not _colour_order_is_uniform(chi_pos, chi_pairs), (name, chi_pos, chi_pairs)
+
+
+# ------------------------------------------------------------------ which occupant of an active cell is tried (a3, S12)
+def _occupant_pick_histogram(L_, sweeps=1500):
+    """Cells two depletant-widened diameters wide hold several spheres (q = 1: w ~ 2 sigma_c).  n_R = 0 and a tiny step,
+    so a sweep only records WHO was tried (outcome code != 0).  hist[k][s] = how often the s-th occupant (ascending
+    particle id) of a k-occupied cell was the one tried; also checks that every non-empty cell tries exactly one."""
+    import ctypes as C
+    import dataclasses
+    from oracle import binding
+    cfg = dataclasses.replace(workloads.config("C1"), N=520, phi_c=0.15, q=1.0, d_max=0.01)
+    pos, _ = workloads.generate(cfg)
+    pos = np.ascontiguousarray(pos, np.float32).copy()
+    par = binding.make_params("sphere", cfg.sigma_c, cfg.sigma_d, cfg.box_L, cfg.d_max)
+    h = L_.oracle_create(C.byref(par), cfg.N, pos.ctypes.data, None)
+    assert h
+    nc, w = C.c_int32(), C.c_float()
+    L_.oracle_grid(h, C.byref(nc), C.byref(w))
+    ncell = nc.value ** 3
+    cs, cp, sh = np.empty(ncell + 1, np.uint32), np.empty(cfg.N, np.uint32), np.empty(3, np.float32)
+    out = np.empty(cfg.N, np.uint8)
+    hist = np.zeros((8, 8), np.int64)
+    for s in range(sweeps):
+        assert L_.oracle_build_cells(h, 5, s) == 0
+        L_.oracle_cells(h, cs.ctypes.data, cp.ctypes.data, sh.ctypes.data)
+        assert L_.oracle_sweep(h, 5, s, 0.0, cfg.d_max, 0.0, 0) == 0
+        L_.oracle_outcomes(h, out.ctypes.data)
+        counts = np.diff(cs.astype(np.int64))
+        cell_of_entry = np.repeat(np.arange(ncell), counts)
+        slot = np.arange(cfg.N) - cs[cell_of_entry].astype(np.int64)
+        tried = out[cp] != 0
+        per_cell = np.bincount(cell_of_entry, weights=tried, minlength=ncell)
+        assert np.array_equal(per_cell, (counts > 0).astype(np.float64)), "a non-empty cell tries exactly one occupant"
+        k = np.minimum(counts[cell_of_entry], 7)
+        np.add.at(hist, (k[tried], np.minimum(slot[tried], 7)), 1)
+    L_.oracle_destroy(h)
+    return hist
+
+
+def _pick_is_uniform(hist):
+    ok, seen = True, 0
+    for k in (2, 3, 4):
+        n = int(hist[k].sum())
+        if n < 5000:
+            continue
+        seen += 1
+        f = hist[k, :k] / n
+        ok = ok and bool(np.all(np.abs(f - 1.0 / k) < 4.0 * math.sqrt((1.0 / k) * (1 - 1.0 / k) / n)))
+    assert seen == 3, hist
+    return ok
+
+
+def test_occupant_of_an_active_cell_is_picked_uniformly():
+    """a3 / S12 pin (north_star "in each active cell one colloid gets a trial"): in cells with k = 2, 3, 4
+    occupants each occupant is the one tried with frequency 1/k within 4 sigma, over ~3 x 10^5 cell visits."""
+    hist = _occupant_pick_histogram(oracle.lib())
+    assert hist[1, 0] == hist[1].sum() and hist[2:5].sum() > 10 ** 5
+    assert _pick_is_uniform(hist), hist[:5, :5]
+
+
+def test_occupant_pick_pin_rejects_always_the_first(tmp_path):
+    L_ = _mutant_library(tmp_path, "first_occupant", "c.cell_pid[b + mulhi32(rs.v[0], nocc)]", "c.cell_pid[b]")
+    assert not _pick_is_uniform(_occupant_pick_histogram(L_, 300) * 5)
 
 
 def test_self_axis_rotation_always_accepted():
