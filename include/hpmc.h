@@ -37,7 +37,8 @@ typedef enum {
   HPMC_SPHERODISK = 2, /* Minkowski sum of a flat disk (radius disk_a, normal z_body) and a ball (radius disk_s) */
   HPMC_TETRAHEDRON = 4, /* regular tetrahedron with circumradius sigma_c / 2, body-frame vertices (sigma_c / (2 sqrt 3)) x
                           {(1,1,1), (1,-1,-1), (-1,1,-1), (-1,-1,1)} (Fig. 1 L21; NEXT-2, reading R-N2b) */
-  HPMC_ELLIPSOID = 3,  /* oblate spheroid, semi-axes (disk_a, disk_a, disk_s), disk_a >= disk_s > 0, short axis z_body: the paper's
+  HPMC_ELLIPSOID = 3,  /* oblate spheroid, semi-axes (disk_a, disk_a, disk_s), 4 disk_s >= disk_a >= disk_s > 0 (aspect ratio at
+                          most 4: what the fixed-length closest-point iteration resolves), short axis z_body: the paper's
                           discoids (reading R-N2); sigma_c must equal 2 disk_a */
   HPMC_SHAPE_COUNT = 5
 } hpmc_shape;
@@ -48,7 +49,11 @@ typedef enum {
   HPMC_E_GEOMETRY = -2,          /* fewer than 4 cells per axis: box too small for the interaction range */
   HPMC_E_STATE = -3,             /* hpmc_sweep without hpmc_build_cells for the same (seed, step) */
   HPMC_E_DMAX = -4,              /* d_max > d_max_cap given at init */
-  HPMC_E_CUDA = -5,              /* CUDA runtime error (message in hpmc_last_error) */
+  HPMC_E_CUDA = -5,              /* CUDA runtime error (message in hpmc_last_error).  Also: in the one-launch sweep a CTA
+                                    waited longer than 60 s of wall clock for a neighbouring CTA's pass -- which the
+                                    cooperative launch rules out short of a lost CTA -- and abandoned the sweep without
+                                    committing the rest of its moves; reported and cleared like the overflow below,
+                                    poses and counters of that sweep are invalid, the context stays usable */
   HPMC_E_NEIGHBOR_OVERFLOW = -6  /* ONE move has more neighbours inside the list radius than the staging buffer holds
                                     (reported and cleared by the next synchronising call; poses of that sweep are
                                     then invalid).  Locally dense tiles do not raise it: the move kernel halves a
@@ -78,7 +83,10 @@ typedef struct {
   uint64_t dep_drawn;       /* sum of N_d over moves that reached the depletant stage (L67) */
   uint64_t dep_needed;      /* sum of (index of the first rejecting depletant + 1), or N_d if none: the
                                sequential algorithm's work; identical in the oracle */
-  uint64_t dep_evaluated;   /* depletant positions the kernel actually generated (>= dep_needed) */
+  uint64_t dep_evaluated;   /* depletant positions the kernel actually generated (>= dep_needed).  This one and
+                               philox_blocks describe the kernel's own work, not the algorithm's: a tile that is
+                               split and redone (neighbour-pool overflow) or a configurational-bias window that is
+                               redone (job overflow) is counted again, so both depend on the tiling */
   uint64_t cb_reinsertions; /* 2 n_trial per rejecting depletant handled (Sec. III.D); 2 n_trial - 1 with HPMC_OPT_ROSENBLUTH */
   uint64_t philox_blocks;   /* Philox4x32-10 blocks computed (warp-uniform ones counted once) */
 } hpmc_counters_t;

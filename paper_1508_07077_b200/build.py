@@ -22,21 +22,26 @@ NVCC_FLAGS = [
 ]
 
 
-def stale() -> bool:
-    if not os.path.exists(SO):
+def stale(so: str = SO) -> bool:
+    if not os.path.exists(so):
         return True
-    t = os.path.getmtime(SO)
+    t = os.path.getmtime(so)
     return any(os.path.getmtime(d) > t for d in DEPS)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if force or stale():
+def build(force: bool = False, verbose: bool = False, defines: tuple = (), out: str | None = None) -> str:
+    """Compile the library if a source is newer than it.  `defines` + `out`: another build of the same sources under
+    another file name (a test build with e.g. HPMC_WAIT_LIMIT_NS=1000, loaded through HPMC_LIBRARY_PATH); the default
+    build takes no defines."""
+    so = SO if out is None else out
+    assert out is not None or not defines, "the default library is built without -D overrides"
+    if force or stale(so):
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        tmp = SO + ".tmp%d" % os.getpid()
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp, SRC]
+        tmp = so + ".tmp%d" % os.getpid()
+        cmd = [nvcc] + NVCC_FLAGS + ["-D" + d for d in defines] + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp, SRC]
         subprocess.run(cmd, check=True)
-        os.replace(tmp, SO)
-    return SO
+        os.replace(tmp, so)
+    return so
 
 
 if __name__ == "__main__":

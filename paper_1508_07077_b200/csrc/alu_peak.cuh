@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(AK_THREADS) k_alu_peak(int iters, uint32_t a, 
         if (KIND == AK_FADD) f[c] = f[c] + fb;
         if (KIND == AK_FMUL) f[c] = f[c] * fb;
         if (KIND == AK_FFMA) f[c] = fmaf(f[c], fb, fa);
-        if (KIND == AK_IMAD) x[c] = x[c] * a + b;
+        if (KIND == AK_IMAD) asm("mad.lo.u32 %0, %0, %1, %2;" : "+r"(x[c]) : "r"(a), "r"(b));   // opaque to the compiler: x a^4 + k cannot be folded
         if (KIND == AK_IMADW_XOR) {               // one Philox half-round: wide multiply, then hi ^ lo ^ key (2 instructions)
           const unsigned long long w = (unsigned long long)x[c] * 0xD2511F53u;
           x[c] = (uint32_t)(w >> 32) ^ (uint32_t)w ^ b;

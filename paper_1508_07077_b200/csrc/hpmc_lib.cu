@@ -3,7 +3,9 @@
 // Per sweep:
 //   hpmc_build_cells: host draws the grid shift from Philox(seed, step, SWEEP) -> K-A kernels (cells.cuh)
 //   hpmc_sweep:       host draws the colour permutation, builds/caches the Poisson threshold table (fp64, R-S2)
-//                     -> 8 launches of the move kernel (move.cuh), one per sub-lattice, stream ordered.
+//                     -> ONE cooperative launch of the item-queue move kernel (moveq.cuh) for the 8 sub-lattice passes;
+//                     the warp-per-cell kernel (move.cuh: configurational bias with few reinsertions on small systems,
+//                     or HPMC_MOVE_KERNEL=warp) takes 8 launches, one per pass, stream ordered.
 // No host synchronisation inside a sweep; no CPU fallback anywhere.
 #include <cuda_runtime.h>
 
@@ -369,6 +371,10 @@ int hpmc_init(hpmc_ctx** out, const hpmc_params* p, int64_t N, float* d_pos4, fl
     if (!(p->disk_s > 0.0f) || !(p->disk_a >= p->disk_s) ||
         std::fabs((double)p->sigma_c - 2.0 * (double)p->disk_a) > 1e-5 * (double)p->sigma_c)
       return fail(nullptr, HPMC_E_BADARG, "hpmc_init: ellipsoid needs disk_a >= disk_s > 0 and sigma_c == 2 disk_a");
+    // the depletant test finds the closest point of the ellipse with a FIXED six Newton steps (geometry.cuh): converged to
+    // fp32 rounding for aspect ratios up to 4, off by up to 1e-4 of a diameter at 10
+    if (p->disk_a > 4.0f * p->disk_s)
+      return fail(nullptr, HPMC_E_BADARG, "hpmc_init: ellipsoid aspect ratio disk_a / disk_s above 4 is not supported");
   }
   if (p->shape == HPMC_SPHERODISK) {
     // sigma_c is the circumsphere diameter 2 (a + s): the insertion radius, the cell width and the list radius derive from it
@@ -415,7 +421,7 @@ int hpmc_init(hpmc_ctx** out, const hpmc_params* p, int64_t N, float* d_pos4, fl
   CUI(cudaMalloc(&ctx->d_cell_start, sizeof(uint32_t) * (padded + SCAN_TILE)));
   CUI(cudaMalloc(&ctx->d_tile_sums, sizeof(uint32_t) * (size_t)ctx->ntiles));
   CUI(cudaMalloc(&ctx->d_outcome, (size_t)N));
-  CUI(cudaMalloc(&ctx->d_counters, sizeof(unsigned long long) * C_COUNT));
+  CUI(cudaMalloc(&ctx->d_counters, sizeof(unsigned long long) * (C_COUNT + 1)));   // + 1: the tally of hpmc_free_volume
   CUI(cudaMalloc(&ctx->d_err, sizeof(int)));
   CUI(cudaMemsetAsync(ctx->d_outcome, 0, (size_t)N, ctx->stream));
   CUI(cudaMemsetAsync(ctx->d_counts, 0, sizeof(uint32_t) * padded, ctx->stream));   // kept zero between builds by k_scan_apply
@@ -599,7 +605,7 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
         case HPMC_ELLIPSOID: rc2 = cb ? launch_moveq<SH_ELLIPSOID, true>(ctx, a, pt, p8) : launch_moveq<SH_ELLIPSOID, false>(ctx, a, pt, p8); break;
         default: rc2 = cb ? launch_moveq<SH_TETRAHEDRON, true>(ctx, a, pt, p8) : launch_moveq<SH_TETRAHEDRON, false>(ctx, a, pt, p8); break;
       }
-      if (rc2) return rc2;
+      if (rc2) { if (ep) --ctx->ev_used; return rc2; }    // no half-recorded event pair for hpmc_move_kernel_ms
     }
     if (one) nlaunch = 1;
   } else {
@@ -615,7 +621,11 @@ int hpmc_sweep(hpmc_ctx* ctx, uint32_t seed, uint32_t step, double n_R, float d_
       }
     }
   }
-  if (ep) { CU(cudaEventRecord(ep->b, ctx->stream)); ep->n = nlaunch; }
+  if (ep) {
+    const cudaError_t eb = cudaEventRecord(ep->b, ctx->stream);
+    if (eb != cudaSuccess) { --ctx->ev_used; return fail(ctx, HPMC_E_CUDA, std::string("cudaEventRecord: ") + cudaGetErrorString(eb)); }
+    ep->n = nlaunch;
+  }
   ctx->launches += nlaunch;
   CU(cudaGetLastError());
   ctx->built = false;
@@ -626,8 +636,9 @@ int hpmc_free_volume(hpmc_ctx* ctx, uint32_t seed, uint32_t step, int64_t n_samp
   if (!ctx || !host_free_count || n_samples < 0) return HPMC_E_BADARG;
   if (!ctx->built || ctx->b_seed != seed || ctx->b_step != step)
     return fail(ctx, HPMC_E_STATE, "hpmc_free_volume: call hpmc_build_cells(seed, step) first");
-  unsigned long long* d_cnt = nullptr;
-  CU(cudaMalloc(&d_cnt, sizeof(unsigned long long)));
+  // the tally lives behind the context's counters: no allocation per measurement, and no cudaFree (which waits for the
+  // whole device)
+  unsigned long long* d_cnt = ctx->d_counters + C_COUNT;
   CU(cudaMemsetAsync(d_cnt, 0, sizeof(unsigned long long), ctx->stream));
   if (n_samples > 0) {
     const Key10 key = make_key(seed, step);
@@ -648,7 +659,6 @@ int hpmc_free_volume(hpmc_ctx* ctx, uint32_t seed, uint32_t step, int64_t n_samp
   CU(cudaMemcpyAsync(&h, d_cnt, sizeof(h), cudaMemcpyDeviceToHost, ctx->stream));
   CU(cudaStreamSynchronize(ctx->stream));
   CU(cudaGetLastError());
-  CU(cudaFree(d_cnt));
   *host_free_count = (uint64_t)h;
   return HPMC_OK;
 }
@@ -677,7 +687,9 @@ static int check_err_flag(hpmc_ctx* ctx) {
   CU(cudaStreamSynchronize(ctx->stream));
   if (e == 2) {
     CU(cudaMemsetAsync(ctx->d_err, 0, sizeof(int), ctx->stream));
-    return fail(ctx, HPMC_E_CUDA, "move kernel: a CTA waited too long for a neighbouring CTA's pass (poses of that sweep are invalid)");
+    return fail(ctx, HPMC_E_CUDA, "move kernel: a CTA waited longer than the wall-clock limit (60 s in the default build) for a "
+                                  "neighbouring CTA's pass and abandoned the sweep without committing its remaining moves "
+                                  "(poses and counters of that sweep are invalid)");
   }
   if (e) {
     CU(cudaMemsetAsync(ctx->d_err, 0, sizeof(int), ctx->stream));
@@ -751,12 +763,24 @@ int hpmc_step_host(hpmc_ctx* ctx, float* host_pos4, float* host_quat4, uint8_t* 
     // sparse download: the device keeps the list of the particles accepted in the sweep; if it is short, only their
     // poses come back and are patched into the host arrays (which hold the uploaded poses of all the others)
     ctx->acc_cap = (size_t)std::max<int64_t>(1, N / 4);
-    CU(cudaMalloc(&ctx->d_acc_count, sizeof(uint32_t)));
-    CU(cudaMalloc(&ctx->d_acc_list, sizeof(uint32_t) * (size_t)N));
-    CU(cudaMalloc(&ctx->d_acc_pack, sizeof(float4) * 2 * ctx->acc_cap));
-    CU(cudaMallocHost(&ctx->h_acc_list, sizeof(uint32_t) * ctx->acc_cap));
-    CU(cudaMallocHost(&ctx->h_acc_pack, sizeof(float4) * 2 * ctx->acc_cap));
-    CU(cudaMallocHost(&ctx->h_acc_count, sizeof(uint32_t)));
+    // all six or none: a failure half-way (the pinned buffers are the likely ones) must not leave d_acc_list set,
+    // or the next call would skip this block and use the missing ones
+    cudaError_t ea = cudaMalloc(&ctx->d_acc_count, sizeof(uint32_t));
+    if (ea == cudaSuccess) ea = cudaMalloc(&ctx->d_acc_pack, sizeof(float4) * 2 * ctx->acc_cap);
+    if (ea == cudaSuccess) ea = cudaMallocHost(&ctx->h_acc_list, sizeof(uint32_t) * ctx->acc_cap);
+    if (ea == cudaSuccess) ea = cudaMallocHost(&ctx->h_acc_pack, sizeof(float4) * 2 * ctx->acc_cap);
+    if (ea == cudaSuccess) ea = cudaMallocHost(&ctx->h_acc_count, sizeof(uint32_t));
+    if (ea == cudaSuccess) ea = cudaMalloc(&ctx->d_acc_list, sizeof(uint32_t) * (size_t)N);
+    if (ea != cudaSuccess) {
+      cudaFree(ctx->d_acc_count); cudaFree(ctx->d_acc_pack); cudaFree(ctx->d_acc_list);
+      if (ctx->h_acc_list) cudaFreeHost(ctx->h_acc_list);
+      if (ctx->h_acc_pack) cudaFreeHost(ctx->h_acc_pack);
+      if (ctx->h_acc_count) cudaFreeHost(ctx->h_acc_count);
+      ctx->d_acc_count = ctx->d_acc_list = ctx->h_acc_list = ctx->h_acc_count = nullptr;
+      ctx->d_acc_pack = ctx->h_acc_pack = nullptr;
+      cudaGetLastError();
+      return fail(ctx, HPMC_E_CUDA, std::string("hpmc_step_host: staging buffers: ") + cudaGetErrorString(ea));
+    }
   }
   int rc = hpmc_upload(ctx, host_pos4, host_quat4);
   if (rc) return rc;
@@ -845,9 +869,13 @@ int hpmc_alu_peaks(hpmc_alu_peaks_t* out, void* cuda_stream) {
   const int grid = 2 * sms;                       // 2 CTAs x 512 threads = 32 warps per SM, one wave
   unsigned long long* d_cyc = nullptr;
   uint32_t* d_sink = nullptr;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  struct Release {                                // frees on every return path, the CU() ones included
+    unsigned long long*& cyc; uint32_t*& sink; cudaEvent_t &a, &b;
+    ~Release() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); cudaFree(cyc); cudaFree(sink); }
+  } release{d_cyc, d_sink, e0, e1};
   CU(cudaMalloc(&d_cyc, sizeof(unsigned long long) * grid));
   CU(cudaMalloc(&d_sink, sizeof(uint32_t)));
-  cudaEvent_t e0, e1;
   CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
   const Key10 key = make_key(1u, 2u);
   std::vector<unsigned long long> cyc((size_t)grid);
@@ -881,8 +909,6 @@ int hpmc_alu_peaks(hpmc_alu_peaks_t* out, void* cuda_stream) {
     out->rate[kind] = best;
   }
   out->sm_mhz_during = mhz_sum;
-  cudaEventDestroy(e0); cudaEventDestroy(e1);
-  cudaFree(d_cyc); cudaFree(d_sink);
   return HPMC_OK;
 }
 

@@ -289,7 +289,7 @@ __global__ void __launch_bounds__(MOVE_WARPS * 32) k_move(const MoveArgs A) {
         nnb += __popc(km);
       }
       if (nnb > MAXNB) {
-        if (lane == 0) atomicExch(A.err_flag, 1);
+        if (lane == 0) atomicMax(A.err_flag, 1);
         nnb = MAXNB;
       }
       __syncwarp();

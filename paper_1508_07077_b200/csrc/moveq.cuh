@@ -73,6 +73,12 @@ __device__ __forceinline__ float sym_unit_bits(uint32_t x) {
 #ifndef HPMC_WALK_DEFER
 #define HPMC_WALK_DEFER 1
 #endif
+// One-launch sweep: how long (wall clock, %globaltimer) a CTA waits for a neighbouring CTA's pass before it abandons the
+// sweep with error code 2 (HPMC_E_CUDA).  Not a tuning knob: the cooperative launch makes every wait finite, so this only
+// turns a lost CTA into an error instead of a hang.  (The abandon path is tested with a build that sets it to microseconds.)
+#ifndef HPMC_WAIT_LIMIT_NS
+#define HPMC_WAIT_LIMIT_NS 60000000000ull
+#endif
 #ifndef HPMC_WALK_SLOTS
 #define HPMC_WALK_SLOTS 4         // phase 1b: particle loads in flight per (move, row) item
 #endif
@@ -125,6 +131,9 @@ struct QSmem {
   // configurational bias (a9): per move the product so far, the rejecting depletants handled, the window start, the
   // head of its job list; per job (one rejecting depletant of the current window) k, move | next, packed counts
   static constexpr int JCAP = CB ? 4 * T : 0;
+  // the job-overflow redo of the CB stage halves the window down to one depletant per move and relies on "one job per
+  // move always fits": without this a larger CPT (HPMC_QCPT) would make that loop spin for ever
+  static_assert(!CB || M <= JCAP, "configurational bias: a tile must not hold more moves than job slots");
   static constexpr size_t o_P = o_nbmap + 4 * NBMAP_WORDS;                       // float[M]
   static constexpr size_t o_cbre = o_P + (CB ? 4 * M : 0);                       // u32[M] jobs counted (x 2 n_trial = reinsertions)
   static constexpr size_t o_klo = o_cbre + (CB ? 4 * M : 0);                     // u32[M]
@@ -350,6 +359,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
   // registers; the per-move ones go to CTA totals in shared memory (far below 2^32)
   uint32_t n_eval = 0, n_blocks = 0;
   if (t < C_COUNT) s_cnt[t] = 0u;               // ordered before the first use by the barrier at the top of the tile loop
+  if (t == 0) s_scal[6] = 0u;                   // "a neighbour wait timed out", likewise
 
   // CTA b owns the active-cell indices [cta_first[b], cta_first[b+1]) for every colour; the host table gives the
   // first-launched CTAs a larger share (the SM's warp arbitration favours them; see setup_moveq).
@@ -388,6 +398,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
   }
 
   uint32_t tile_cap = (uint32_t)Q.tile_cells;     // halved (for the rest of this CTA's share) when a tile's neighbour pool overflows
+  bool gave_up = false;                           // a neighbour wait ran into HPMC_WAIT_LIMIT_NS (CTA-uniform)
 #pragma unroll 1
   for (int pass = 0; pass < Q.npass; ++pass) {
   const uint32_t colour = Q.npass > 1 ? Q.colours[pass] : A.colour;
@@ -467,7 +478,11 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
     // ---- passes after the first: the neighbourhood walk reads cells that neighbouring CTAs wrote in the previous
     // pass (and they must be done reading ours): wait for their published pass counter.  Acquire loads by the
     // polling threads + the barrier make their writes visible to the whole CTA.  Phase 1a above touched only this
-    // CTA's own cells, so it ran ahead of the wait.  Bounded spin: a stuck neighbour raises the error flag instead of a hang.
+    // CTA's own cells, so it ran ahead of the wait.  The launch is cooperative, so the neighbour is resident and WILL
+    // publish, however slow its pass is (n_trial up to 65535, a clustered share, a debugger): the wait is not bounded in
+    // polls.  The wall-clock bound (HPMC_WAIT_LIMIT_NS, looked at every 4096 polls) only guards against a lost CTA, and
+    // when it strikes this CTA does not go on against cells its neighbour may still be writing: it raises the error
+    // flag and abandons the rest of the sweep (see "gave_up" below).
     HPMC_PHASE_MARK(1);        // phase 1a (thread 0's own share of it)
     if (must_wait) {
       must_wait = false;
@@ -476,10 +491,16 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
       for (uint32_t b = (uint32_t)t; b < gridDim.x; b += T) {
         if (!((s_nbmap[b >> 5] >> (b & 31)) & 1u)) continue;
         uint32_t v, spins = 0;
+        unsigned long long t_first = 0ull;
         for (;;) {       // relaxed polls (no L1 invalidation while spinning), one acquire fence at the end
           asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(Q.done + b) : "memory");
           if ((int32_t)(v - target) >= 0) break;
-          if (++spins > (1u << 20)) { atomicExch(A.err_flag, 2); break; }
+          if ((++spins & 4095u) == 0u) {
+            unsigned long long now;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+            if (t_first == 0ull) t_first = now;
+            else if (now - t_first > (unsigned long long)(HPMC_WAIT_LIMIT_NS)) { atomicMax(A.err_flag, 2); s_scal[6] = 1u; break; }
+          }
           __nanosleep(spins < 64u ? 40u : 200u);      // short waits are the rule (small systems are latency-bound); back off on long ones
         }
         polled = true;
@@ -487,6 +508,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
       if (polled) asm volatile("fence.acq_rel.gpu;" ::: "memory");
     }
     __syncthreads();
+    if (Q.npass > 1 && s_scal[6]) { gave_up = true; break; }      // nothing of this tile is committed
     HPMC_PHASE_MARK(2);        // neighbour wait + barrier after 1a
     const int nlist = (int)s_scal[4];
 
@@ -587,7 +609,7 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
     // committed yet (boundary outcomes are idempotent, its counters are tile-local), so halve the tile and redo it
     if (s_scal[1] > (uint32_t)POOL) {
       if (tile_n > 1u) { tile_cap = max(1u, tile_n >> 1); cur = tile_lo; __syncthreads(); continue; }
-      if (t == 0) atomicExch(A.err_flag, 1);     // ONE move with more listed neighbours than the whole pool holds
+      if (t == 0) atomicMax(A.err_flag, 1);      // ONE move with more listed neighbours than the whole pool holds
     }
     // ================================================================ phase 1d: N_d by table inversion (a7)
 #pragma unroll 1
@@ -777,15 +799,16 @@ __global__ void __launch_bounds__(T, (CB ? 1 : QLayout<SHAPE>::MIN_CTAS * (T < 1
     HPMC_PHASE_MARK(6);        // commit + barrier
   }
   // ---- publish the pass: every commit of this CTA is ordered before the counter by the barrier above + the release
+  // (a CTA without cells in this pass has nothing to wait for: it reads and writes no cell.)  A CTA that gave up
+  // publishes the counter's end-of-sweep value at once, so that no neighbour waits for passes it will never run and the
+  // host's sequence number stays valid for the next sweep; the poses of this sweep are invalid and the flag says so.
   if (Q.npass > 1) {
-    if (must_wait) {      // a CTA without cells in this pass still has to respect the order of its neighbours' passes: nothing to do
-      must_wait = false;
-    }
     if (t == 0) {
-      const uint32_t v = Q.seq0 + (uint32_t)pass + 1u;
+      const uint32_t v = Q.seq0 + (uint32_t)(gave_up ? Q.npass : pass + 1);
       asm volatile("st.release.gpu.global.u32 [%0], %1;" :: "l"(Q.done + blockIdx.x), "r"(v) : "memory");
     }
   }
+  if (gave_up) break;
   }   // pass
 
   // ---- counters: REDUX for the two register counters, then one global atomic per CTA and counter
