@@ -736,6 +736,9 @@ struct oracle_params {
 void* oracle_create(const oracle_params* p, int64_t N, float* pos4, float* quat4) {
   if (!p || N <= 0 || !pos4 || !(p->box_L > 0.0f) || !(p->sigma_c > 0.0f) || p->sigma_d < 0.0f) return nullptr;
   if (p->shape != SH_SPHERE && !quat4) return nullptr;
+  // near_spheroid's six Newton steps resolve the point-to-ellipse distance to fp32 rounding for aspect ratios up to 4
+  // (pinned at 2 and at 4); flatter discoids would need more steps, so they are refused rather than answered loosely
+  if (p->shape == SH_ELLIPSOID && !(p->disk_s > 0.0f && p->disk_a >= p->disk_s && p->disk_a <= 4.0f * p->disk_s)) return nullptr;
   Ctx* c = new Ctx();
   c->g = make_geo(p->shape, p->sigma_c, p->disk_a, p->disk_s, p->sigma_d, p->box_L, p->d_max_cap);
   c->N = N; c->pos = pos4; c->quat = quat4;

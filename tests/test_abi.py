@@ -79,6 +79,9 @@ def test_no_gpu_means_loud_failure_not_fallback(lib):
     assert lib.hpmc_init(C.byref(ctx), C.byref(p), 0, None, None, None) == -1
     small = binding.Params(0, 1.0, 0.0, 0.0, 0.1, 4.0, 0.05)
     assert lib.hpmc_init(C.byref(ctx), C.byref(small), 10, None, None, None) == -2  # HPMC_E_GEOMETRY
+    flat = binding.Params(3, 1.0, 0.5, 0.1, 0.1, 20.0, 0.05)                        # ellipsoid, aspect ratio 5 > 4
+    assert lib.hpmc_init(C.byref(ctx), C.byref(flat), 10, None, None, None) == -1
+    assert b"aspect" in lib.hpmc_last_error(None)
     if torch.cuda.is_available():
         pytest.skip("a GPU is present: the no-device branch cannot be exercised")
     rc = lib.hpmc_init(C.byref(ctx), C.byref(p), 10, None, None, None)

@@ -178,6 +178,40 @@ def test_dilated_volume_and_contacts_tetrahedron(olib):
         assert pair_overlap(TE, [-t, -t, -t], ident, ident)[0] == (gap < 0)
 
 
+def test_ellipsoid_depletant_test_at_the_largest_aspect_ratio(olib):
+    """R-N2: the closest point of the ellipse comes from a fixed six Newton steps, so accuracy depends on the aspect
+    ratio; 4 is the largest the library and the oracle accept.  At A = 0.5, C = 0.125 the predicate must agree with the
+    distance from a root finder (scipy brentq on F(t), fp64) for every point farther than 2e-6 from the decision surface,
+    for a small, a matching and a large depletant; aspect 5 is refused."""
+    from scipy.optimize import brentq
+    A, Cc = 0.5, 0.125
+    rng = np.random.default_rng(21)
+    for sigma_d in (0.06, 0.25, 1.0):
+        par = dict(EL, disk_s=Cc, sigma_d=sigma_d)
+        rd, R = 0.5 * sigma_d, 0.5 + 0.5 * sigma_d
+        pts = (rng.random((6000, 3)) * 2 - 1) * R
+        rho, z = np.hypot(pts[:, 0], pts[:, 1]), np.abs(pts[:, 2])
+        dist = np.zeros(len(pts))
+        for k in range(len(pts)):
+            if (rho[k] / A) ** 2 + (z[k] / Cc) ** 2 <= 1.0:
+                continue
+            F = lambda t: (A * rho[k] / (t + A * A)) ** 2 + (Cc * z[k] / (t + Cc * Cc)) ** 2 - 1.0
+            lo = max(A * rho[k] - A * A, Cc * z[k] - Cc * Cc)
+            t = brentq(F, lo, lo + 100.0, xtol=1e-15)
+            dist[k] = math.hypot(rho[k] - A * A * rho[k] / (t + A * A), z[k] - Cc * Cc * z[k] / (t + Cc * Cc))
+        want = (dist < rd) & (np.linalg.norm(pts, axis=1) < R)
+        got = dep_overlap(par, np.array([1, 0, 0, 0], np.float32), pts)
+        clear = (np.abs(dist - rd) > 2e-6) & (np.abs(np.linalg.norm(pts, axis=1) - R) > 2e-6)
+        assert clear.sum() > 5900 and want[clear].sum() > 500 and (~want[clear]).sum() > 500
+        assert np.array_equal(got[clear], want[clear]), (sigma_d, int((got[clear] != want[clear]).sum()))
+    p4 = np.zeros((1, 4), np.float32); p4[0, :3] = 5.0
+    q4 = np.array([[1, 0, 0, 0]], np.float32)
+    ok = olib.oracle_create(C.byref(make_params(**dict(EL, disk_s=0.125))), 1, p4.ctypes.data, q4.ctypes.data)
+    assert ok
+    olib.oracle_destroy(ok)
+    assert not olib.oracle_create(C.byref(make_params(**dict(EL, disk_s=0.1))), 1, p4.ctypes.data, q4.ctypes.data)
+
+
 def test_pair_overlap_closed_forms_ellipsoid():
     """Coaxial spheroids overlap iff |dz| < 2 C; coplanar ones (same axis, separation in the equatorial plane) iff the
     distance is < 2 A; an edge-on spheroid above a flat one (axes perpendicular) iff the gap is < A + C."""
