@@ -42,6 +42,14 @@ OPS_PER_MOVE = {"sphere": 500.0,                  # 3 Philox blocks, 27-cell wal
                 "halfball": 1500.0,               # + axis staging, ~2 support-function pair tests of ~400 ops (a6)
                 "spherodisk": 1500.0, "ellipsoid": 1500.0, "tetrahedron": 2000.0}
 OPS_PER_CB_REINSERTION = {"sphere": 150.0, "halfball": 190.0, "spherodisk": 190.0, "ellipsoid": 440.0, "tetrahedron": 520.0}   # 1.91 x 62 + both pose tests + neighbour tests
+# INT / FP32 split of the same totals (lower bound = max(FP / FP rate, INT / INT rate, all / issue rate,
+# bytes / HBM)).  Integer work does not depend on the shape: per cube-rejection attempt one Philox block (20 wide
+# multiplies + 20 three-input XORs) + 3 bit operations of the bits->float conversion = 43, x 6/pi attempts = 82 per needed
+# depletant or reinsertion; per move 3 Philox blocks (120) + ~80 of row addressing and table search = 200.  The rest of
+# each total is non-FMA FP32 (differences, products, compares of the overlap tests).  The totals above stay as frozen.
+INT_OPS_PER_NEEDED_DEPLETANT = 82.0
+INT_OPS_PER_CB_REINSERTION = 82.0
+INT_OPS_PER_MOVE = 200.0
 PHILOX_BLOCKS_PER_DEPLETANT = 6.0 / 3.141592653589793
 BYTES_PER_PARTICLE_PER_PASS = 16.0 # every pass reads the cell-ordered float4 array once (re-reads by neighbouring cells are L2 hits)
 BYTES_PER_CELL_PER_PASS = 4.0      # ... and each cell_start word once
@@ -157,11 +165,11 @@ def reduce_over_ranks(total_ms, work, device, world):
     return float(t.item()), [float(x) for x in w.tolist()]
 
 
-def oracle_sample(cfg, pos, quat, sweeps, step0, min_seconds=0.0, max_sweeps=None):
-    """Time the CPU oracle, as it stands, on `sweeps` sweeps of the same workload with all host cores; with
-    min_seconds > 0 keep adding sweeps until that much CPU wall time has been spent (bounded by max_sweeps)."""
+def oracle_sample(cfg, pos, quat, sweeps, step0, min_seconds=0.0, max_sweeps=None, threads=None):
+    """Time the CPU oracle, as it stands, on `sweeps` sweeps of the same workload with all host cores (or `threads`);
+    with min_seconds > 0 keep adding sweeps until that much CPU wall time has been spent (bounded by max_sweeps)."""
     import oracle
-    threads = os.cpu_count() or 1
+    threads = threads or os.cpu_count() or 1
     o = oracle.Oracle(cfg.shape, cfg.sigma_c, cfg.sigma_d, cfg.box_L, cfg.d_max, pos, quat, cfg.disk_a, cfg.disk_s,
                       threads=threads)
     times = []
@@ -230,10 +238,17 @@ def roofline_block(cfg, c, n_c, passes, launches, kernel_ms, step_ms_total, alu,
                  + moves * BYTES_PER_MOVE + (c["accept_trans"] + c["accept_rot"]) * BYTES_PER_ACCEPT)
     kernel_s = kernel_ms * 1e-3
     sms, hz = alu["num_sms"], pk["sm_max_mhz"] * 1e6
+    int_ops = (c["dep_needed"] * INT_OPS_PER_NEEDED_DEPLETANT + moves * INT_OPS_PER_MOVE
+               + c["cb_reinsertions"] * INT_OPS_PER_CB_REINSERTION)
+    fp_ops = alg_ops - int_ops
     t_philox = blocks / (alu["philox_blocks_ilp4"] * sms * hz)
     t_issue = alg_ops / (alu["fadd_lop3_mix"] * sms * hz)
+    t_fp = fp_ops / (min(alu["fadd"], alu["fmul"]) * sms * hz)                 # non-FMA FP32 stream
+    t_int = int_ops / (alu["imadwide_lop3_pair"] * sms * hz)                   # IMAD.WIDE + LOP3 stream (the Philox mix)
     t_hbm = alg_bytes / (pk["hbm_gbs"] * 1e9)
-    t_alu = max(t_philox, t_issue)
+    terms = {"fp32": t_fp, "int": t_int, "issue": t_issue, "philox_blocks": t_philox, "hbm": t_hbm}
+    binding = max(("fp32", "int", "issue", "philox_blocks"), key=lambda k: terms[k])
+    t_alu = terms[binding]
     peak = alg_ops / t_alu
     ach = alg_ops / kernel_s if kernel_s > 0 else 0.0
     hbm_ach = alg_bytes / kernel_s / 1e9 if kernel_s > 0 else 0.0
@@ -251,10 +266,16 @@ def roofline_block(cfg, c, n_c, passes, launches, kernel_ms, step_ms_total, alu,
         "achieved": ach / 1e12, "peak": peak / 1e12, "unit": "Tlaneop/s", "frac": t_alu / kernel_s if kernel_s > 0 else None,
         "frac_cycles": (t_alu * hz) / (kernel_s * seen_mhz * 1e6) if kernel_s > 0 else None,
         "traffic": traffic, "traffic_source": traffic_src,
-        "peak_source": "measured live: hpmc_alu_peaks on this device (per SM per clock: %.3f Philox blocks, %.1f lane-ops two-pipe "
-                       "issue) x %d SMs x %.0f MHz; binding term: %s; HBM %s" % (
-                           alu["philox_blocks_ilp4"], alu["fadd_lop3_mix"], sms, pk["sm_max_mhz"],
-                           "philox pipe" if t_philox >= t_issue else "issue", pk["source"]),
+        "peak_source": "measured live: hpmc_alu_peaks on this device (per SM per clock: %.1f FP32 non-FMA, %.1f IMAD.WIDE+LOP3, "
+                       "%.1f two-pipe issue lane-ops, %.3f Philox blocks) x %d SMs x %.0f MHz; binding term: %s; HBM %s" % (
+                           min(alu["fadd"], alu["fmul"]), alu["imadwide_lop3_pair"], alu["fadd_lop3_mix"],
+                           alu["philox_blocks_ilp4"], sms, pk["sm_max_mhz"], binding, pk["source"]),
+        # time lower bound = max over the pipes; every term in microseconds per launch, and the fraction the
+        # combined-issue term alone gives (the only ALU term of the round-1 and round-2 lines, kept for comparison)
+        "binding_term": binding,
+        "terms_us_per_launch": {k: 1e6 * v / max(1, launches) for k, v in terms.items()},
+        "frac_issue_term_only": t_issue / kernel_s if kernel_s > 0 else None,
+        "alg_int_laneops_per_launch": int_ops / max(1, launches), "alg_fp32_laneops_per_launch": fp_ops / max(1, launches),
         "peak_issue_bound": issue_peak / 1e12, "frac_of_issue_bound": ach / issue_peak,
         "alg_laneops_per_launch": alg_ops / max(1, launches), "alg_philox_blocks_per_launch": blocks / max(1, launches),
         "alg_bytes_per_launch": alg_bytes / max(1, launches),
@@ -428,6 +449,33 @@ def main():
         total_ms, [moves, c["dep_evaluated"], c["dep_needed"], c["dep_drawn"]], "cuda", world)
     tot_s = job_ms * 1e-3
 
+    # ---- SURVEY 8(d) / BASELINE.md 3: the same sweep repeated from IDENTICAL initial poses (identical work every time),
+    # median of the event times; `value` above stays the base contract's K consecutive sweeps of one trajectory
+    reps = None
+    if world == 1:
+        n_rep, n_skip = 7, 2
+        pos_ref = torch.from_numpy(pos.copy()).cuda()
+        quat_ref = None if quat is None else torch.from_numpy(quat.copy()).cuda()
+        h.reset_counters()
+        ra = [torch.cuda.Event(enable_timing=True) for _ in range(n_rep + n_skip)]
+        rb = [torch.cuda.Event(enable_timing=True) for _ in range(n_rep + n_skip)]
+        for r in range(n_rep + n_skip):
+            dpos.copy_(pos_ref)
+            if dquat is not None:
+                dquat.copy_(quat_ref)
+            flush.zero_()
+            ra[r].record()
+            step(0)
+            rb[r].record()
+        torch.cuda.synchronize()
+        cr = h.counters()
+        rep_ms = sorted(a.elapsed_time(b) for a, b in zip(ra[n_skip:], rb[n_skip:]))
+        rep_moves = (cr["trials_trans"] + cr["trials_rot"]) / (n_rep + n_skip)
+        med = statistics.median(rep_ms)
+        reps = {"n": n_rep, "untimed_first": n_skip, "sweep": "step 0 from the seeded initial poses, poses restored before every repetition",
+                "ms_median": med, "ms_min": rep_ms[0], "ms_max": rep_ms[-1], "moves_per_repetition": rep_moves,
+                "moves_per_s_median": rep_moves / (med * 1e-3)}
+
     # ---- e2e: the same step through the host-buffer C-ABI call, copies inside the timed region
     e2e = None
     if not args.no_e2e:
@@ -470,6 +518,11 @@ def main():
             cpu = {"value": om / sum(times), "unit": "moves/s", "cores": threads, "kind": "oracle",
                    "sample": "%d sweeps of the same workload from the same initial poses (%.1f s)" % (ns, sum(times)),
                    "dep_needed_per_s": oc["dep_needed"] / sum(times)}
+            # the same oracle on ONE core (SURVEY 8(d) "Oracle timing" (i)): two sweeps from the same initial poses
+            _, oc1, t1, th1 = oracle_sample(cfg, pos, quat, 2, args.warmup, threads=1)
+            cpu["single_thread"] = {"value": (oc1["trials_trans"] + oc1["trials_rot"]) / sum(t1), "unit": "moves/s",
+                                    "cores": th1, "dep_needed_per_s": oc1["dep_needed"] / sum(t1),
+                                    "sample": "%d sweeps (%.1f s)" % (len(t1), sum(t1))}
         line = {
             "metric": "colloid_trial_moves_per_s", "value": g_moves / tot_s, "unit": "moves/s", "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": job_ms / args.steps,
@@ -481,6 +534,7 @@ def main():
             "acceptance": (c["accept_trans"] + c["accept_rot"]) / max(1, moves),
             "roofline": roofline, "alu_peaks_per_sm_per_clk": alu, "cpu_baseline": cpu, "e2e": e2e,
             "gpu_launches": launches, "clocks": clocks, "per_config": per_config, "wall_s_timed_region": t_wall,
+            "repetitions": reps,
         }
         print(json.dumps(line), flush=True)
     h.close()
